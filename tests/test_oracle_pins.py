@@ -1,0 +1,349 @@
+"""Pins for the float64 oracle (oracle/himuon_oracle.py) against what the paper and the
+mathematics fix -- NOT against itself.  CPU only (`-m "not gpu"`).
+
+Each test names the passage (PAPER.md line + section) or the closed form it relies on.
+"""
+import math
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from oracle import himuon_oracle as O
+
+A_, B_, C_ = 3.4445, -4.7750, 2.0315   # retyped from PAPER.md:74 on purpose
+
+
+def rng(seed):
+    return np.random.default_rng(seed)
+
+
+def scalar_iterate(x, K, a=A_, b=B_, c=C_):
+    """f_K: K-fold iterate of p(x) = a x + b x^3 + c x^5 (the action of Eq. 2.2 on a singular value)."""
+    for _ in range(K):
+        x = a * x + b * x ** 3 + c * x ** 5
+    return x
+
+
+# ----------------------------------------------------------------------------- golden: paper constants
+
+def test_coefficients_match_paper(paper_numbers):
+    # PAPER.md:74 Eq. (2.3)
+    assert O.NS_A == float(paper_numbers["ns_a"])
+    assert O.NS_B == float(paper_numbers["ns_b"])
+    assert O.NS_C == float(paper_numbers["ns_c"])
+    assert O.HParams().scale_c == float(paper_numbers["scale_c"])
+    assert O.HParams().K == 5 and O.HParams().beta == 0.95
+
+
+# ----------------------------------------------------------------------------- Phi_K
+
+@pytest.mark.parametrize("H,W", [(8, 8), (6, 17), (17, 6), (32, 48)])
+def test_svd_closed_form(H, W):
+    """Phi_K(U S V^T) = U f_K(S / ||S||_2) V^T: Eq. (2.2) acts on each singular value by the odd
+    polynomial p; checked through numpy's SVD, independent of the matmul recurrence."""
+    A = rng(1).standard_normal((H, W))
+    U, s, Vt = np.linalg.svd(A, full_matrices=False)
+    for K in (0, 1, 3, 5):
+        want = (U * scalar_iterate(s / np.linalg.norm(s), K)) @ Vt
+        got = O.phi(A, K=K)
+        assert np.max(np.abs(got - want)) < 1e-12
+
+
+def test_svd_closed_form_with_eps():
+    # reading Q2: eps is added to the Frobenius norm
+    A = rng(2).standard_normal((12, 20)) * 1e-3
+    eps = 1e-4
+    U, s, Vt = np.linalg.svd(A, full_matrices=False)
+    want = (U * scalar_iterate(s / (np.linalg.norm(s) + eps), 5)) @ Vt
+    assert np.max(np.abs(O.phi(A, eps=eps) - want)) < 1e-12
+    assert np.max(np.abs(O.phi(A, eps=0.0) - want)) > 1e-3      # eps must matter here
+
+
+def test_one_step_against_expanded_polynomial():
+    """One NS step written the other way round: X1 = a X + b (X X^T) X + c (X X^T)(X X^T) X,
+    evaluated with explicit triple loops on a tiny matrix (brute force)."""
+    A = rng(3).standard_normal((3, 4))
+    X = A / math.sqrt(sum(v * v for v in A.ravel()))
+    H, W = X.shape
+    G = [[sum(X[i, k] * X[j, k] for k in range(W)) for j in range(H)] for i in range(H)]
+    G2 = [[sum(G[i][k] * G[k][j] for k in range(H)) for j in range(H)] for i in range(H)]
+    X1 = np.zeros((H, W))
+    for i in range(H):
+        for j in range(W):
+            X1[i, j] = A_ * X[i, j] + sum((B_ * G[i][k] + C_ * G2[i][k]) * X[k, j] for k in range(H))
+    assert np.max(np.abs(O.phi(A, K=1) - X1)) < 1e-14
+
+
+def test_transpose_equivariance():
+    # H > W applies the recurrence to A^T and transposes back
+    A = rng(4).standard_normal((24, 10))
+    assert np.array_equal(O.phi(A.T), O.phi(A).T)
+    # and the row / column oriented recurrences agree (reading Q7)
+    X = A / np.linalg.norm(A)
+    for _ in range(5):
+        Gc = X.T @ X
+        X = X @ (A_ * np.eye(10) + B_ * Gc + C_ * Gc @ Gc)
+    assert np.max(np.abs(O.phi(A) - X)) < 1e-13
+
+
+def test_zero_and_oddness_and_scale_invariance():
+    Z = np.zeros((5, 7))
+    assert np.array_equal(O.phi(Z), Z)
+    assert np.array_equal(O.phi(Z, eps=1e-7), Z)
+    A = rng(5).standard_normal((9, 9))
+    assert np.array_equal(O.phi(-A), -O.phi(A))              # odd polynomial
+    assert np.max(np.abs(O.phi(37.5 * A) - O.phi(A))) < 1e-13   # X0 normalised
+
+
+def test_orthogonal_invariance():
+    A = rng(6).standard_normal((10, 14))
+    Q, _ = np.linalg.qr(rng(7).standard_normal((10, 10)))
+    P, _ = np.linalg.qr(rng(8).standard_normal((14, 14)))
+    assert np.max(np.abs(O.phi(Q @ A @ P) - Q @ O.phi(A) @ P)) < 1e-13
+
+
+def test_semi_orthogonal_input():
+    """A with orthonormal rows (H <= W): all singular values 1, ||A||_F = sqrt(H), so
+    Phi_K(A) = f_K(1/sqrt(H)) A.  (Basis of the RMS argument of PAPER.md:153.)"""
+    H, W = 20, 33
+    Q, _ = np.linalg.qr(rng(9).standard_normal((W, H)))
+    A = Q.T
+    want = scalar_iterate(1.0 / math.sqrt(H), 5) * A
+    assert np.max(np.abs(O.phi(A) - want)) < 1e-13
+
+
+def test_T1_exact_rational():
+    """T = 1: every 1x1 tile x maps to sign(x) f_K(1); f_K(1) evaluated in exact rational
+    arithmetic from the decimal coefficients of PAPER.md:74 (f_1(1) = a+b+c = 0.7010)."""
+    a, b, c = Fraction("3.4445"), Fraction("-4.7750"), Fraction("2.0315")
+    x = Fraction(1)
+    vals = []
+    for _ in range(5):
+        x = a * x + b * x ** 3 + c * x ** 5
+        vals.append(x)
+    assert vals[0] == Fraction("0.7010")
+    A = rng(10).standard_normal((4, 6))
+    A[1, 2] = 0.0
+    got = O.phi_tiled(A, 1)
+    want = np.sign(A) * float(vals[4])
+    assert abs(float(vals[4]) - 0.696436409469752) < 1e-12   # SURVEY.md 8(c) value, by hand
+    assert np.max(np.abs(got - want)) < 1e-14
+    assert got[1, 2] == 0.0
+    for K in range(1, 6):
+        assert np.max(np.abs(O.phi_tiled(A, 1, K=K) - np.sign(A) * float(vals[K - 1]))) < 1e-14
+
+
+def test_K0_returns_normalised_input():
+    A = rng(11).standard_normal((7, 5))
+    assert np.max(np.abs(O.phi(A, K=0) - A / np.linalg.norm(A))) < 1e-16
+
+
+# ----------------------------------------------------------------------------- B_T, Phi_{K,T}
+
+def test_tile_grid_and_padding():
+    # PAPER.md:48-53
+    assert O.tile_grid(1600, 6400, 128) == (13, 50)
+    assert O.tile_grid(256, 512, 64) == (4, 8)               # reading Q1: 32 tiles, not 8
+    A = np.arange(5 * 7, dtype=np.float64).reshape(5, 7) + 1
+    t = O.tile(A, 4)
+    assert t.shape == (2, 2, 4, 4)
+    assert np.array_equal(t[0, 0], A[:4, :4])
+    assert np.array_equal(t[1, 1][:1, :3], A[4:, 4:])
+    assert np.all(t[1, 1][1:, :] == 0) and np.all(t[1, 1][:, 3:] == 0)
+    assert np.all(t[0, 1][:, 3:] == 0) and np.array_equal(t[0, 1][:, :3], A[:4, 4:])
+    assert np.array_equal(O.untile(t, 5, 7), A)              # B_T^{-1} B_T = id
+
+
+def test_T_ge_max_is_full_map():
+    # R = C = 1 and the tiled map coincides with the full-matrix map
+    A = rng(12).standard_normal((12, 20))
+    full = O.phi(A)
+    for T in (20, 21, 64, None):
+        assert np.array_equal(O.phi_tiled(A, T), full)
+    # a single zero-PADDED square tile gives the same values (padding invariance)
+    P = np.zeros((32, 32)); P[:12, :20] = A
+    out = O.phi(P)
+    assert np.max(np.abs(out[:12, :20] - full)) < 1e-13
+    assert np.all(out[12:, :] == 0) and np.all(out[:, 20:] == 0)
+
+
+def test_tiled_differs_from_full():
+    # PAPER.md:142-143, Eq. (4.4)
+    A = rng(13).standard_normal((16, 16))
+    assert np.max(np.abs(O.phi_tiled(A, 8) - O.phi(A))) > 1e-2
+
+
+def test_ragged_equals_unpadded_block():
+    """Edge tiles: Phi_K of the zero-padded tile, cropped, equals Phi_K of the unpadded ragged
+    block; padded region stays exactly zero."""
+    H, W, T = 21, 30, 8
+    A = rng(14).standard_normal((H, W))
+    out = O.phi_tiled(A, T)
+    R, C = O.tile_grid(H, W, T)
+    for r in range(R):
+        for c in range(C):
+            blk = A[r * T:min(H, (r + 1) * T), c * T:min(W, (c + 1) * T)]
+            want = O.phi(blk)
+            got = out[r * T:min(H, (r + 1) * T), c * T:min(W, (c + 1) * T)]
+            assert np.max(np.abs(got - want)) < 1e-13
+    tiles = O.tile(A, T)
+    pad_out = O.phi(tiles[R - 1, C - 1])
+    assert np.all(pad_out[H - (R - 1) * T:, :] == 0.0)
+    assert np.all(pad_out[:, W - (C - 1) * T:] == 0.0)
+
+
+def test_tile_independence():
+    # tiles are processed in isolation
+    H, W, T = 24, 40, 8
+    A = rng(15).standard_normal((H, W))
+    base = O.phi_tiled(A, T)
+    A2 = A.copy()
+    A2[9, 19] += 0.5                                         # inside tile (1, 2)
+    out = O.phi_tiled(A2, T)
+    mask = np.zeros((H, W), dtype=bool)
+    mask[8:16, 16:24] = True
+    assert np.array_equal(out[~mask], base[~mask])           # bitwise elsewhere
+    assert np.max(np.abs(out[mask] - base[mask])) > 1e-4
+
+
+def test_block_diagonal_tile_aligned():
+    T = 6
+    blocks = [rng(16 + i).standard_normal((T, T)) for i in range(3)]
+    A = np.zeros((3 * T, 3 * T))
+    for i, b in enumerate(blocks):
+        A[i * T:(i + 1) * T, i * T:(i + 1) * T] = b
+    out = O.phi_tiled(A, T)
+    for i in range(3):
+        for j in range(3):
+            blk = out[i * T:(i + 1) * T, j * T:(j + 1) * T]
+            if i == j:
+                assert np.array_equal(blk, O.phi(blocks[i]))
+            else:
+                assert np.all(blk == 0.0)
+
+
+def test_phi_tiles_packed_matches_tiled():
+    A = rng(20).standard_normal((16, 24))
+    t = O.tile(A, 8)
+    packed = t.reshape(-1, 8, 8)
+    out = O.phi_tiles(packed).reshape(t.shape)
+    assert np.array_equal(O.untile(out, 16, 24), O.phi_tiled(A, 8))
+
+
+def test_output_statistics_band():
+    """128x128 N(0,1) tile: singular values of Phi_5 land in the band the scalar map allows for
+    inputs sigma/||sigma|| in (0, 0.2]; entry RMS * sqrt(T) is O(1)."""
+    A = rng(21).standard_normal((128, 128))
+    s = np.linalg.svd(O.phi(A), compute_uv=False)
+    # max of f_5 on [0, 1] is about 1.2024; a square Gaussian tile has a few near-zero singular
+    # values (hard edge), which f_5 amplifies by at most a^5 = 484.9 but need not lift into the band
+    assert s.max() < 1.21 and np.mean((s > 0.6) & (s < 1.21)) > 0.95
+    rms = math.sqrt(np.mean(O.phi(A) ** 2)) * math.sqrt(128)
+    assert 0.7 < rms < 1.1
+
+
+# ----------------------------------------------------------------------------- Algorithm 4.1
+
+def test_tau():
+    # PAPER.md:153-166
+    assert O.tau(4096, 14336, 128) == pytest.approx(0.2 * math.sqrt(128))
+    assert O.tau(100, 60, 128) == pytest.approx(0.2 * math.sqrt(100))
+    assert O.tau(100, 60, None) == pytest.approx(0.2 * math.sqrt(100))
+    assert O.tau(128, 128, 128) == pytest.approx(0.2 * math.sqrt(128))   # T >= max -> full branch
+    assert O.tau(1600, 1600, 128, 0.5) == pytest.approx(0.5 * math.sqrt(128))
+
+
+def test_momentum_forms():
+    G = rng(22).standard_normal((4, 5)); M0 = rng(23).standard_normal((4, 5))
+    M, Gh = O.momentum(G, M0, 0.9, True)
+    assert np.allclose(M, 0.9 * M0 + G, rtol=0, atol=1e-15)
+    assert np.allclose(Gh, G + 0.9 * (0.9 * M0 + G), rtol=0, atol=1e-15)  # PAPER.md:94 (new M_t)
+    M, Gh = O.momentum(G, M0, 0.9, False)
+    assert np.array_equal(Gh, M)                                          # Alg. 4.1 l.8-9
+
+
+def test_step_identities():
+    H, W, T = 16, 24, 8
+    r = rng(24)
+    Wt, G, M0 = r.standard_normal((H, W)), r.standard_normal((H, W)), r.standard_normal((H, W))
+    hp = O.HParams(lr=0.0, wd=0.3)
+    Wn, M, U = O.step(Wt, G, M0, hp, T)
+    assert np.array_equal(Wn, Wt)                                        # eta = 0
+    hp = O.HParams(beta=0.0)
+    Wn, M, U = O.step(Wt, G, M0, hp, T)
+    assert np.array_equal(M, G) and np.array_equal(U, O.phi_tiled(G, T))  # beta = 0
+    hp = O.HParams(lr=0.02, wd=0.0)
+    Wn, M, U = O.step(Wt, G, np.zeros_like(G), hp, T)
+    # first step, M_0 = 0: Ghat = (1+beta) G, and Phi is scale invariant
+    assert np.max(np.abs(U - O.phi_tiled(G, T))) < 1e-13
+    assert np.max(np.abs((Wt - Wn) - 0.02 * 0.2 * math.sqrt(T) * U)) < 1e-15   # Eq. (4.6), lambda = 0
+    hp = O.HParams(lr=0.02, wd=0.01)
+    Wn2, _, U2 = O.step(Wt, G, M0, hp, T)
+    assert np.max(np.abs(Wn2 - ((1 - 0.02 * 0.01) * Wt - 0.02 * O.tau(H, W, T) * U2))) < 1e-15
+    # full branch inside step: T >= max(H, W) uses tau = c sqrt(max(H,W)) and the full map
+    Wn3, _, U3 = O.step(Wt, G, M0, hp, 64)
+    _, Gh = O.momentum(G, M0, hp.beta, True)
+    assert np.array_equal(U3, O.phi(Gh))
+    assert np.max(np.abs(Wn3 - ((1 - 0.02 * 0.01) * Wt - 0.02 * 0.2 * math.sqrt(24) * U3))) < 1e-15
+
+
+def test_momentum_independent_of_T():
+    # optimizer state is independent of the tile size
+    r = rng(25)
+    Wt, G, M0 = r.standard_normal((16, 16)), r.standard_normal((16, 16)), r.standard_normal((16, 16))
+    hp = O.HParams()
+    Ms = [O.step(Wt, G, M0, hp, T)[1] for T in (4, 8, 16, None)]
+    for M in Ms[1:]:
+        assert np.array_equal(M, Ms[0])
+
+
+# ----------------------------------------------------------------------------- planner (paper's worked example)
+
+def _shapes(s):
+    return [tuple(int(v) for v in tok.split("x")) for tok in s.split()]
+
+
+def test_planner_paper_numbers(paper_numbers):
+    """PAPER.md:390, :398 and Table 2: 28 blocks x 7 matrices = 196 calls;
+    Qwen3-0.6B at T=512 has 1680 tiles (one call); Qwen3-1.7B has 5376 tiles -> 2 chunks of 2688."""
+    nb = int(paper_numbers["qwen3_blocks"]); T = int(paper_numbers["tile_size"])
+    s06 = _shapes(paper_numbers["shapes_0p6b"]) * nb
+    s17 = _shapes(paper_numbers["shapes_1p7b"]) * nb
+    assert len(s17) == int(paper_numbers["unbatched_calls_1p7b"])
+    w06 = O.enumerate_tiles(s06, [T] * len(s06))
+    w17 = O.enumerate_tiles(s17, [T] * len(s17))
+    assert len(w06) == int(paper_numbers["tiles_0p6b"])
+    assert len(w17) == int(paper_numbers["tiles_1p7b"])
+    # staged model of the paper: in + out bf16 per tile; any cap admitting 2688..5375 tiles gives 2 x 2688
+    bpt = 2 * T * T * 2
+    for cap_tiles in (2688, 3000, 5375):
+        offs = O.chunk_offsets(len(w17), bpt, cap_tiles * bpt)
+        assert len(offs) - 1 == int(paper_numbers["chunks_1p7b"])
+        assert offs[1] - offs[0] == offs[2] - offs[1] == int(paper_numbers["chunk_size_1p7b"])
+    assert len(O.chunk_offsets(len(w06), bpt, 2688 * bpt)) - 1 == int(paper_numbers["chunks_0p6b"])
+
+
+def test_enumerate_order_and_full_branch():
+    w = O.enumerate_tiles([(5, 9), (4, 4), (3, 3)], [4, 4, 8])
+    assert w[:6] == [(0, 0, 0), (0, 0, 1), (0, 0, 2), (0, 1, 0), (0, 1, 1), (0, 1, 2)]
+    assert w[6] == (1, 0, 0)          # T >= max(H,W): single entry
+    assert w[7] == (2, 0, 0) and len(w) == 8
+
+
+def test_chunk_offsets_balanced_and_fewest():
+    offs = O.chunk_offsets(10, 8, 8 * 4)        # at most 4 per chunk -> 3 chunks 4,3,3
+    assert offs == [0, 4, 7, 10]
+    assert O.chunk_offsets(0, 8, 64) == [0]
+    assert O.chunk_offsets(7, 0, 0) == [0, 7]
+    assert O.chunk_offsets(7, 8, 1000, fixed_bytes=1000 - 16) == [0, 2, 4, 6, 7]
+    with pytest.raises(ValueError):
+        O.chunk_offsets(3, 8, 4)
+
+
+def test_per_tile_error_metric():
+    A = rng(30).standard_normal((8, 8))
+    Bm = A.copy(); Bm[0:4, 4:8] *= 1.1
+    e = O.per_tile_rel_fro_error(Bm, A, 4)
+    assert e.shape == (2, 2)
+    assert e[0, 1] == pytest.approx(0.1) and e[0, 0] == 0 and e[1, 1] == 0

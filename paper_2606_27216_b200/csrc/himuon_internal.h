@@ -1,0 +1,93 @@
+// Internal declarations shared by the host planner, the C-ABI dispatch and the kernels.
+// Not part of the public boundary (that is include/himuon.h).
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "himuon.h"
+
+namespace himuon {
+
+// ---- device-visible tables (live in the caller's workspace) ---------------------------------
+
+// One layer of the descriptor table, 64 bytes.
+struct LayerDev {
+  void*     w;
+  void*     g;
+  void*     m;
+  long long ld_w, ld_g, ld_m;   // elements
+  int       H, W;
+  float     tau_base;           // sqrt(T) or sqrt(max(H,W)) (full branch); tau = scale_c * tau_base
+  int       dtype;              // himuon_dtype
+};
+static_assert(sizeof(LayerDev) == 64, "LayerDev must be 64 bytes");
+
+// One entry of the cross-layer work list: tile (r, c) of layer `layer`.
+struct WorkItem {
+  int layer, r, c, pad;
+};
+static_assert(sizeof(WorkItem) == 16, "WorkItem must be 16 bytes");
+
+enum Mode : int { MODE_STEP = 0, MODE_PHI = 1 };
+enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1 };
+
+struct LaunchArgs {
+  const LayerDev*    layers;     // device
+  const CUtensorMap* tmaps;      // device, 3 per layer (w, g, m); may be null on the SIMT path
+  const WorkItem*    items;      // device; null => implicit list: item i = (layer 0, r = i, c = 0)
+  long long          n_items;
+  int                T;
+  int                mode;
+  int                dtype;      // storage dtype of every layer in this launch (bucket key)
+  himuon_hparams     hp;
+};
+
+// kernels_simt.cu -- fp32 FMA path, T in {16, 32, 64, 128}, fp32 or bf16 storage.
+cudaError_t launch_simt(const LaunchArgs& a, cudaStream_t stream);
+// kernels_tc128.cu -- tcgen05 bf16 path, T = 128, bf16 storage.
+cudaError_t launch_tc128(const LaunchArgs& a, cudaStream_t stream);
+
+int  device_sm_count();
+void note_launch();
+
+// ---- host plan --------------------------------------------------------------------------------
+
+struct Bucket {
+  int       T;
+  int       dtype;
+  int       kpath;
+  long long begin, end;   // range in the work list
+};
+
+struct Chunk {
+  int       bucket;
+  long long begin, end;
+};
+
+}  // namespace himuon
+
+struct himuon_plan {
+  std::vector<himuon_layer>     layers;
+  std::vector<int>              T_eff;       // per layer, effective (supported) tile size
+  std::vector<int>              kpath;       // per layer
+  std::vector<himuon::LayerDev> layer_dev;
+  std::vector<himuon::WorkItem> items;       // execution order
+  std::vector<himuon::Bucket>   buckets;
+  std::vector<himuon::Chunk>    chunks;
+  bool      resident  = true;                // whole list fits under the cap
+  bool      bindable  = true;                // all pointers non-null
+  bool      needs_tma = false;
+  size_t    fixed_bytes = 0;                 // layer table + tensor maps
+  size_t    off_tmaps = 0, off_items = 0;
+  long long max_chunk_tiles = 0;
+  size_t    workspace_bytes = 0;
+  size_t    cap = 0;
+  // binding
+  void*             ws = nullptr;
+  himuon::WorkItem* pinned_items = nullptr;  // streaming mode only
+};

@@ -1,0 +1,170 @@
+"""CPU-only tests of the C-ABI library's host logic: it loads, exports every symbol declared in
+include/himuon.h, validates arguments, and its planner (work list, buckets, memory-bounded
+chunking) agrees with the oracle's enumeration and with the numbers the paper prints."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import himuon_inputs as I
+import paper_2606_27216_b200 as hm
+from paper_2606_27216_b200 import binding as B
+from paper_2606_27216_b200.build import build
+from oracle import himuon_oracle as O
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build()
+
+
+def _layers(shapes, dtype=hm.HIMUON_BF16, Ts=None):
+    return [hm.himuon_layer(hm.shape_mat(h, w, dtype), hm.shape_mat(h, w, dtype), hm.shape_mat(h, w, dtype),
+                            0 if Ts is None else Ts[i]) for i, (h, w) in enumerate(shapes)]
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "himuon.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(himuon_[a-z0-9_]+)\s*\(", hdr))
+    assert {"himuon_plan_create", "himuon_step", "himuon_phi", "himuon_ns_tiles", "himuon_plan_bind"} <= names
+    lib = C.CDLL(B.LIB_PATH)
+    for n in sorted(names):
+        assert hasattr(lib, n), f"libhimuon.so does not export {n}"
+
+
+def test_status_strings():
+    lib = B._lib()
+    assert lib.himuon_status_string(0) == b"HIMUON_OK"
+    assert lib.himuon_status_string(2) == b"HIMUON_ERR_UNSUPPORTED"
+
+
+@pytest.mark.parametrize("shapes,T", [([(256, 512)], 64), ([(1600, 1600), (1600, 6400), (6400, 1600)], 128),
+                                      ([(100, 90), (33, 700)], 32), ([(5, 3)], 16)])
+def test_worklist_matches_oracle_enumeration(shapes, T):
+    """R = ceil(H/T), C = ceil(W/T); layer order then r-major."""
+    p = hm.Plan(_layers(shapes), T)
+    lrc, offs, cT = p.worklist()
+    want = O.enumerate_tiles(shapes, [T] * len(shapes))
+    assert [tuple(x) for x in lrc.tolist()] == want
+    assert p.n_tiles == len(want) and p.n_buckets == 1 and p.n_chunks == 1
+    assert offs.tolist() == [0, len(want)]
+
+
+def test_config1_tile_count_reading_Q1():
+    # 256x512 at T=64 is 4 x 8 = 32 tiles by PAPER.md:48-49 (BASELINE's "8 tiles" is T=128)
+    assert hm.Plan(_layers([(256, 512)], hm.HIMUON_F32), 64).n_tiles == 32
+    assert hm.Plan(_layers([(256, 512)], hm.HIMUON_F32), 128).n_tiles == 8
+
+
+def test_tile_counts_of_the_benchmark_configs():
+    # SURVEY.md 8(a) [derived]: config 2 = 5184, config 4 = 94848, config 5 = 425984 tiles at T=128
+    for spec, n in ((I.gpt2_small_spec(), 5184), (I.gpt2_xl_spec(), 94848), (I.llama3_8b_spec(), 425984)):
+        p = hm.Plan(_layers([(l.H, l.W) for l in spec.layers]), 128)
+        assert p.n_tiles == n
+        assert p.n_chunks == 1
+
+
+def test_paper_planner_numbers(paper_numbers):
+    """1680 tiles -> 1 call; 5376 tiles -> two chunks of 2688 (T=512)."""
+    T = int(paper_numbers["tile_size"])
+    blocks = int(paper_numbers["qwen3_blocks"])
+
+    def n_tiles(key):
+        shapes = [tuple(int(x) for x in s.split("x")) for s in paper_numbers[key].split()]
+        return blocks * sum(-(-h // T) * -(-w // T) for h, w in shapes)
+
+    n06, n17 = n_tiles("shapes_0p6b"), n_tiles("shapes_1p7b")
+    assert n06 == int(paper_numbers["tiles_0p6b"]) and n17 == int(paper_numbers["tiles_1p7b"])
+    per_tile = 3 * T * T * 2                      # paper's staged model: in + intermediate + out, bf16
+    for cap_tiles in (2688, 3000, 5375):          # any budget admitting 2688..5375 tiles
+        offs = hm.himuon_plan_chunks(n17, per_tile, 0, cap_tiles * per_tile)
+        assert offs == [0, int(paper_numbers["chunk_size_1p7b"]), n17]
+        assert hm.himuon_plan_chunks(n06, per_tile, 0, cap_tiles * per_tile) == [0, n06]
+
+
+@pytest.mark.parametrize("n,per,fixed,cap", [(10, 7, 3, 30), (1000, 16, 1000, 5000), (7, 1, 0, 2), (5, 0, 0, 1), (0, 4, 0, 100)])
+def test_chunk_rule_matches_oracle(n, per, fixed, cap):
+    assert hm.himuon_plan_chunks(n, per, fixed, cap) == O.chunk_offsets(n, per, cap, fixed)
+
+
+def test_chunk_rule_too_small():
+    with pytest.raises(hm.HimuonError) as e:
+        hm.himuon_plan_chunks(10, 100, 0, 50)
+    assert e.value.status == B.HIMUON_ERR_WORKSPACE_TOO_SMALL
+
+
+def test_chunked_plan_is_balanced_and_fewest():
+    shapes = [(1600, 1600)] * 3
+    full = hm.Plan(_layers(shapes), 128)
+    fixed = full.workspace_bytes - full.n_tiles * 16
+    p = hm.Plan(_layers(shapes), 128, workspace_cap_bytes=fixed + 16 * 100)
+    lrc, offs, _ = p.worklist()
+    sizes = np.diff(offs)
+    assert p.n_chunks == -(-full.n_tiles // 100) and sizes.max() - sizes.min() <= 1 and sizes.max() <= 100
+    assert p.workspace_bytes <= fixed + 16 * 100
+    assert [tuple(x) for x in lrc.tolist()] == O.enumerate_tiles(shapes, [128] * 3)   # order unchanged
+
+
+def test_runtime_tile_schedule_buckets():
+    """Reading Q13: per-layer T; tiles bucketed by (T, dtype, path); momentum is not
+    part of the plan, so re-planning cannot touch it."""
+    shapes = [(256, 256), (128, 512), (256, 256), (512, 128)]
+    Ts = [128, 64, 128, 32]
+    p = hm.Plan(_layers(shapes, Ts=Ts), 128)
+    lrc, offs, cT = p.worklist()
+    assert p.n_buckets == 3 and cT.tolist() == [128, 64, 32]
+    want = []
+    for T in (128, 64, 32):
+        want += [x for x in O.enumerate_tiles(shapes, Ts) if Ts[x[0]] == T]
+    assert [tuple(x) for x in lrc.tolist()] == want
+
+
+def test_full_branch_is_one_padded_tile():
+    # T >= max(H,W): R = C = 1; run as the smallest supported tile >= max(H,W)
+    p = hm.Plan(_layers([(100, 90)]), 128)
+    lrc, _, cT = p.worklist()
+    assert lrc.tolist() == [[0, 0, 0]] and cT.tolist() == [128]
+    p = hm.Plan(_layers([(20, 30)], hm.HIMUON_F32), 128)
+    assert p.worklist()[2].tolist() == [32]
+    with pytest.raises(hm.HimuonError) as e:
+        hm.Plan(_layers([(4096, 4096)]), 8192)
+    assert e.value.status == B.HIMUON_ERR_UNSUPPORTED
+
+
+def test_argument_validation():
+    S = B.HIMUON_ERR_INVALID_ARG
+    for bad in ([(0, 5)], [(5, -1)]):
+        with pytest.raises(hm.HimuonError) as e:
+            hm.Plan(_layers(bad), 32)
+        assert e.value.status == S
+    with pytest.raises(hm.HimuonError) as e:      # ld < W
+        hm.Plan([hm.himuon_layer(hm.shape_mat(8, 8, ld=4), hm.shape_mat(8, 8), hm.shape_mat(8, 8), 0)], 16)
+    assert e.value.status == S
+    with pytest.raises(hm.HimuonError) as e:      # T not a supported size
+        hm.Plan(_layers([(256, 256)]), 48)
+    assert e.value.status == S
+    with pytest.raises(hm.HimuonError) as e:      # bad dtype
+        hm.Plan(_layers([(256, 256)], dtype=7), 32)
+    assert e.value.status == S
+    p = hm.Plan(_layers([(256, 256)]), 128)       # unbound / unbindable plan
+    with pytest.raises(hm.HimuonError) as e:
+        p.step(hm.HParams())
+    assert e.value.status == B.HIMUON_ERR_NOT_BOUND
+    lib = B._lib()
+    assert lib.himuon_plan_bind(p._h, None, 0, None) == S
+    assert lib.himuon_ns_tiles(None, None, -1, 32, 0, 0, 5, 1.0, 1.0, 1.0, 0.0, None, 0, None) == S
+    assert lib.himuon_ns_tiles(None, None, 4, 48, 0, 0, 5, 1.0, 1.0, 1.0, 0.0, None, 0, None) == S
+    assert lib.himuon_ns_tiles(None, None, 0, 32, 0, 0, 5, 1.0, 1.0, 1.0, 0.0, None, 0, None) == B.HIMUON_OK
+
+
+def test_tma_alignment_is_checked():
+    # tensor-core path: ld*2 must be a multiple of 16 bytes
+    with pytest.raises(hm.HimuonError) as e:
+        hm.Plan([hm.himuon_layer(hm.himuon_mat(256, 256, 256, 257, 1), hm.himuon_mat(256, 256, 256, 257, 1),
+                                 hm.himuon_mat(256, 256, 256, 257, 1), 0)], 128)
+    assert e.value.status == B.HIMUON_ERR_UNSUPPORTED

@@ -1,0 +1,368 @@
+#!/usr/bin/env python
+"""Benchmark of the HiMuon hot path on B200 (contract: see the task statement / DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload llama3-8b|gpt2-xl|gpt2-small] [--T 128]
+    python bench.py --impl reference ...        # the float64 oracle timed on the host cores
+    python bench.py --suite                     # per-config / per-T table (JSON lines), context lines included
+
+One "step" = one pass of the whole hot path (plan already built; momentum -> tile -> normalise ->
+K Newton-Schulz steps -> untile -> scaled, weight-decayed write) over one parameter set of seeded
+synthetic gradients.  Default workload: BASELINE.json configs[4], the Llama-3-8B-shaped parameter set
+(the configuration the north-star target is quoted on), T = 128, K = 5, bf16 storage.
+Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+import himuon_inputs as I
+
+METRIC = "himuon_step_tiled_ns_tflops"
+UNIT = "TFLOP/s"
+
+
+def spec_of(name: str):
+    if name == "llama3-8b":
+        return I.llama3_8b_spec()
+    if name == "llama3-8b-sched":
+        return I.llama3_8b_spec(schedule=True)
+    if name == "gpt2-xl":
+        return I.gpt2_xl_spec()
+    if name == "gpt2-small":
+        return I.gpt2_small_spec()
+    raise SystemExit(f"unknown workload {name}")
+
+
+def algorithmic_flops(spec, T_default: int, K: int) -> float:
+    """6*K*T*H*W per matrix (Eq. 4.5; BASELINE.json north_star; reading Q16)."""
+    return float(sum(6.0 * K * (l.T or T_default) * l.H * l.W for l in spec.layers))
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_burst": d["bf16_tflops"], "bf16_sustained": d["bf16_tflops_sustained"],
+                "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu, self.proc = gpu_index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.gpu)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, pw, reasons = [], [], [], set()
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# ----------------------------------------------------------------------------- oracle legs (CPU)
+
+def oracle_sample_run(spec, T: int, hp, n_tiles: int, seed: int = 1234):
+    """Time the float64 oracle (as it stands) on a bounded sample of the workload: `n_tiles` T x T
+    tiles cut from freshly drawn layers of the parameter set, one full Algorithm-4.1 step each.
+    Returns (seconds, flops, cores)."""
+    from oracle import himuon_oracle as O
+    ohp = O.HParams(lr=hp.lr, beta=hp.beta, nesterov=bool(hp.nesterov), wd=hp.wd, K=hp.K, a=hp.a, b=hp.b, c=hp.c,
+                    eps=hp.eps, scale_c=hp.scale_c)
+    # draw one T-row strip of a layer per sample group (same recipe as the GPU inputs)
+    tiles, li = [], 0
+    while len(tiles) < n_tiles:
+        l = spec.layers[li % len(spec.layers)]
+        Tl = l.T or T
+        cols = min(l.W, 8 * Tl)
+        G = I.lowrank_plus_noise(Tl, cols, spec.rank, seed_cfg=spec.seed_cfg, layer_index=li, tensor_id=I.TENSOR_G)
+        M = I.lowrank_plus_noise(Tl, cols, spec.rank, seed_cfg=spec.seed_cfg, layer_index=li, tensor_id=I.TENSOR_M)
+        W = I.gaussian(Tl, cols, seed_cfg=spec.seed_cfg, layer_index=li, tensor_id=I.TENSOR_W, dtype=torch.bfloat16, scale=0.02)
+        for c in range(cols // Tl):
+            sl = slice(c * Tl, (c + 1) * Tl)
+            tiles.append((I.to_f64_numpy(W[:, sl]), I.to_f64_numpy(G[:, sl]), I.to_f64_numpy(M[:, sl]), Tl))
+        li += 1
+    tiles = tiles[:n_tiles]
+    t0 = time.perf_counter()
+    flops = 0.0
+    for (W, G, M, Tl) in tiles:
+        O.step(W, G, M, ohp, Tl)   # a T x T block at tile size T is exactly one tile (R = C = 1)
+        flops += 6.0 * hp.K * Tl * Tl * Tl
+    dt = time.perf_counter() - t0
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        cores = 1
+    return dt, flops, cores
+
+
+# ----------------------------------------------------------------------------- GPU arm
+
+def make_inputs(spec, device):
+    Ws, Gs, Ms = [], [], []
+    for i in range(len(spec.layers)):
+        W, G, M = I.make_layer_tensors(spec, i, dtype=torch.bfloat16, device=device)
+        Ws.append(W); Gs.append(G); Ms.append(M)
+    return Ws, Gs, Ms
+
+
+def run_gpu(args):
+    import paper_2606_27216_b200 as hm
+    rank, world, local = dist_env()
+    if args.gpus != world:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("launch multi-GPU runs with torch.distributed.run (one rank per GPU)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    spec = spec_of(args.workload)
+    if args.blocks:
+        per_block = {"llama3-8b": 7, "llama3-8b-sched": 7, "gpt2-xl": 6, "gpt2-small": 6}[args.workload]
+        spec.layers = spec.layers[: per_block * args.blocks]
+        spec.name += f"[first {args.blocks} blocks]"
+    hp = hm.HParams(K=args.K, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
+    Ws, Gs, Ms = make_inputs(spec, dev)                       # weak scaling: every rank owns a full parameter set
+    Tl = [l.T for l in spec.layers]
+    plan = hm.Plan.from_tensors(Ws, Gs, Ms, args.T, T_per_layer=Tl if any(Tl) else None,
+                                workspace_cap_bytes=args.cap_mb << 20).bind()
+    flops = algorithmic_flops(spec, args.T, args.K)
+    n_elem = spec.n_elements
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        plan.step(hp)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = hm.himuon_launch_count()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_begin.record(stream)
+    for k in range(args.steps):
+        evs[k][0].record(stream)
+        plan.step(hp)
+        evs[k][1].record(stream)
+    t_end.record(stream)
+    barrier()
+    launches = hm.himuon_launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = t_begin.elapsed_time(t_end)
+    per_step = [a.elapsed_time(b) for a, b in evs]
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([total_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * flops / (ms_per_step * 1e-3) / 1e12
+
+    # ---- e2e: same metric through the public API with HOST buffers (gradients in, weights out)
+    e2e = run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier)
+
+    if rank != 0:
+        return
+    pk = peaks()
+    kern_ms = statistics.mean(per_step) / max(1, plan.n_chunks)     # dominant kernel = the fused step kernel
+    ach = flops / plan.n_chunks / (kern_ms * 1e-3) / 1e12
+    bytes_step = 10.0 * n_elem
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(f"{args.workload}:T{args.T}")
+    roof = {"bound": "tensor", "achieved": round(ach, 2), "peak": pk["bf16_sustained"], "unit": "TFLOP/s",
+            "frac": round(ach / pk["bf16_sustained"], 4), "traffic": traffic,
+            "peak_kind": "sustained bf16, " + pk["source"], "frac_of_burst": round(ach / pk["bf16_burst"], 4),
+            "kernel": "himuon_tc128_kernel", "launch_ms": round(kern_ms, 4),
+            "hbm_gbs_achieved": round(bytes_step / (ms_per_step * 1e-3) / 1e9, 1), "hbm_frac": round(bytes_step / (ms_per_step * 1e-3) / 1e9 / pk["hbm_gbs"], 4),
+            "roofline_ms": round(max(flops / (pk["bf16_sustained"] * 1e12), bytes_step / (pk["hbm_gbs"] * 1e9)) * 1e3, 3)}
+    cpu = run_cpu_baseline(args, spec, hp)
+    line = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": f"{spec.name}-shaped HiMuon step (BASELINE configs[4])" if spec.name == "llama3-8b" else f"{spec.name}-shaped HiMuon step",
+                       "layers": len(spec.layers), "elements": n_elem, "tiles": plan.n_tiles, "T": args.T, "K": args.K,
+                       "chunks": plan.n_chunks, "workspace_bytes": plan.workspace_bytes, "cap_mb": args.cap_mb,
+                       "l2": "inputs (%.1f GB) larger than L2" % (bytes_step / 1e9), "parallelism": f"replicas x{world}, no collective",
+                       "gflop_per_step": round(flops / 1e9, 1)},
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+            "step_ms_median": round(statistics.median(per_step), 4), "step_ms_min": round(min(per_step), 4)}
+    print(json.dumps(line))
+
+
+def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
+    """Per step: H2D copy of the step's gradients from pinned host memory, himuon_step, D2H read of the
+    updated weights into pinned host memory.  Host buffers are bounded by --e2e-host-gb."""
+    sizes = [g.numel() * 2 for g in Gs]
+    budget = int(args.e2e_host_gb * (1 << 30))
+    n_layers, acc = 0, 0
+    for sz in sizes:                       # both a G-in and a W-out host buffer per layer
+        if acc + 2 * sz > budget:
+            break
+        acc += 2 * sz
+        n_layers += 1
+    n_layers = max(n_layers, 1)
+    full = n_layers == len(Gs)
+    sub_Ws, sub_Gs = Ws[:n_layers], Gs[:n_layers]
+    if full:
+        sub_plan, sub_flops = plan, flops
+    else:
+        Ms_sub = [torch.zeros_like(g) for g in sub_Gs]
+        Tl = [l.T for l in spec.layers[:n_layers]]
+        sub_plan = hm.Plan.from_tensors(sub_Ws, sub_Gs, Ms_sub, args.T, T_per_layer=Tl if any(Tl) else None).bind()
+        sub_flops = float(sum(6.0 * args.K * (l.T or args.T) * l.H * l.W for l in spec.layers[:n_layers]))
+    hG = [torch.empty(g.shape, dtype=g.dtype, pin_memory=True) for g in sub_Gs]
+    hW = [torch.empty(w.shape, dtype=w.dtype, pin_memory=True) for w in sub_Ws]
+    for h, g in zip(hG, sub_Gs):
+        h.copy_(g)
+    steps = max(2, min(args.steps, 5))
+
+    def one():
+        for h, g in zip(hG, sub_Gs):
+            g.copy_(h, non_blocking=True)
+        sub_plan.step(hp)
+        for h, w in zip(hW, sub_Ws):
+            h.copy_(w, non_blocking=True)
+
+    one()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        one()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1) / steps
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    h2d = sum(h.numel() * 2 for h in hG)
+    d2h = sum(h.numel() * 2 for h in hW)
+    return {"value": round(world * sub_flops / (ms * 1e-3) / 1e12, 3), "unit": UNIT, "ms_per_step": round(ms, 3),
+            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": steps,
+            "workload": "full parameter set" if full else f"first {n_layers} of {len(Gs)} layers (host-buffer budget {args.e2e_host_gb} GB)"}
+
+
+def run_cpu_baseline(args, spec, hp):
+    n = args.cpu_tiles
+    dt, fl, cores = oracle_sample_run(spec, args.T, hp, n)
+    return {"value": round(fl / dt / 1e12, 6), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n} tiles of {args.T}x{args.T} (one Algorithm-4.1 step each) drawn with the {spec.name} recipe; "
+                      f"{dt:.1f} s of float64 numpy", "seconds": round(dt, 2)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step = a bounded sample."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    import paper_2606_27216_b200 as hm   # HParams container only; no kernels are called on this arm
+    spec = spec_of(args.workload)
+    hp = hm.HParams(K=args.K, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
+    n = max(8, args.cpu_tiles // 8)
+    for _ in range(args.warmup):
+        oracle_sample_run(spec, args.T, hp, n)
+    tot_t, tot_f, cores = 0.0, 0.0, 1
+    for _ in range(args.steps):
+        dt, fl, cores = oracle_sample_run(spec, args.T, hp, n)
+        tot_t += dt; tot_f += fl
+    v = tot_f / tot_t / 1e12
+    line = {"impl": "reference", "metric": METRIC, "value": round(v, 6), "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(tot_t / args.steps * 1e3, 2),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{spec.name}-shaped HiMuon step, bounded sample of {n} tiles per step", "T": args.T, "K": args.K},
+            "cpu_baseline": {"value": round(v, 6), "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{n} tiles of {args.T}x{args.T} per step, {args.steps} steps"},
+            "e2e": {"value": round(v, 6), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="himuon", choices=["himuon", "reference"])
+    ap.add_argument("--workload", default="llama3-8b")
+    ap.add_argument("--T", type=int, default=128)
+    ap.add_argument("--K", type=int, default=5)
+    ap.add_argument("--cap-mb", type=int, default=2048)
+    ap.add_argument("--cpu-tiles", type=int, default=4096)
+    ap.add_argument("--e2e-host-gb", type=float, default=8.0)
+    ap.add_argument("--blocks", type=int, default=0, help="truncate the parameter set to its first N transformer blocks (profiling only)")
+    ap.add_argument("--suite", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.suite:
+        from bench_suite import run_suite
+        return run_suite(args)
+    run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

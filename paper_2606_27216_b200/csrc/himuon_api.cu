@@ -26,11 +26,15 @@ constexpr size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 const int kTileSizes[] = {16, 32, 64, 128, 256};
 
 // Which kernel serves (dtype, requested path, T); -1 = none in this build.
-int select_kpath(int dtype, int path, int T) {
+// W = number of columns of the matrix (0 = unknown / any).  The TMA stores of the tensor-core path
+// work in 16-byte granules of a row, so a bf16 matrix whose width is not a multiple of 8 is served
+// by the fp32 kernel instead (measured on B200: a store clipped at such a width zero-fills the rest
+// of the last granule, i.e. it would write into the ld - W gutter).
+int select_kpath(int dtype, int path, int T, int W = 0) {
   const bool simt_ok = (T == 16 || T == 32 || T == 64 || T == 128);
   if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : -1;
   // bf16 storage, AUTO: tensor-core path where it exists, else the fp32 kernel.
-  if (T == 128) return KPATH_TC;
+  if (T == 128 && (W % 8) == 0) return KPATH_TC;
   return simt_ok ? KPATH_FP32_SIMT : -1;
 }
 
@@ -206,7 +210,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       if (select_kpath(dt, path, T) < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
       Te = T;
     }
-    const int kp = select_kpath(dt, path, Te);
+    const int kp = select_kpath(dt, path, Te, W);
     p->T_eff[l] = Te;
     p->kpath[l] = kp;
     if (!L.g.ptr || !L.w.ptr) p->bindable = false;

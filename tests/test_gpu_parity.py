@@ -206,7 +206,9 @@ def test_tc128_chunked_equals_unchunked():
     Ws, Gs, Ms = _param_set(shapes, 25)
     hp = hm.HParams(K=5, eps=1e-7, wd=0.01)
     outs = []
-    for cap in (0, 3 * 64 + 128 + 9 * 128 + 16 * 5):
+    probe = hm.Plan.from_tensors(Ws, Gs, Ms, 128)
+    fixed = probe.workspace_bytes - 16 * probe.n_tiles
+    for cap in (0, fixed + 16 * 5):
         Wd, Gd, Md = [w.to(DEV) for w in Ws], [g.to(DEV) for g in Gs], [m.to(DEV) for m in Ms]
         plan = hm.Plan.from_tensors(Wd, Gd, Md, 128, workspace_cap_bytes=cap).bind()
         if cap:

@@ -7,15 +7,18 @@
 // Per tile (Alg. 4.1; Eq. 2.2-2.3; Eq. 4.6), everything between the TMA loads of
 // G, M, W and the TMA stores of M, W stays on chip:
 //   P   TMA G,M -> smem; M' = beta M + G; Ghat = G + beta M' (Nesterov) | M'; M' -> TMA store;
-//       X0 = Ghat / (||Ghat||_F + eps)  -> fp32 in TMEM (state) and bf16 in smem (MMA operand)
-//   K x MMA1  ACC  = Xb Xb^T                                   (A = X X^T)
-//       E1    d = diag(ACC); O = offdiag(ACC); Ob = bf16(O) -> smem;
-//             ACC <- O_ij (b/c + d_i + d_j)  (i != j),  (b/c) d_i + d_i^2  (i == j)
-//       MMA2  ACC += Ob Ob^T                                   (=> ACC = B / c, B = bA + cA^2)
-//       E2    dB_i = c ACC_ii; bf16(c ACC_ij, i != j) -> smem;  X <- (a + dB_i) X   (fp32, TMEM)
-//       MMA3  X += offdiag(B)b Xb                              (=> X = aX + BX)
-//       E3    Xb = bf16(X) -> smem
-//   F   TMA W -> smem; W' = (1 - lr wd) W - lr tau X_K -> TMA store   (Phi mode: store X_K)
+//       Xh0 = q Ghat / (||Ghat||_F + eps), q = c^(1/4)  -> fp32 in TMEM (state), bf16 in smem (operand)
+//       (with the state scaled by q: Ah = Xh Xh^T = sqrt(c) A and B = bA + cA^2 = beta Ah + Ah^2,
+//        beta = b / sqrt(c), so no accumulator ever needs a rescale by c)
+//   K x MMA1  ACC  = Xb Xb^T                                   (Ah)
+//       E1    Ob = bf16(ACC), diagonal zeroed -> smem;  S_t = sum_j ACC_tj^2 = (Ah^2)_tt  (fp32)
+//             ACC <- ACC_ij (beta + d_i + d_j),  d_t = ||Xh row t||^2 = (Ah)_tt  (fp32)
+//       MMA2  ACC += Ob Ob^T                                   (=> ACC_ij = B_ij for i != j)
+//             meanwhile: X <- (a + B_tt) X,  B_tt = beta d_t + S_t          (fp32, TMEM, row scaling)
+//       E2    bf16(ACC), diagonal zeroed -> smem
+//       MMA3  X += offdiag(B)b Xb                              (=> Xh = a Xh + B Xh)
+//       E3    Xb = bf16(X) -> smem;  d_t = sum_j X_tj^2
+//   F   TMA W -> smem; W' = (1 - lr wd) W - lr tau X_K / q -> TMA store   (Phi mode: store X_K / q)
 // The diagonals of A and B (O(1) numbers whose bf16 rounding would dominate the error) never pass
 // through bf16: they act as fp32 row scalings.  DESIGN.md "Numerical scheme" derives the algebra.
 //
@@ -71,17 +74,28 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 __device__ __forceinline__ float bf16_lo(uint32_t u) { return __uint_as_float(u << 16); }
 __device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u & 0xffff0000u); }
 
-// Write 32 fp32 values (columns 32g .. 32g+31 of row r) as bf16 into a swizzled tile.
-__device__ __forceinline__ void store_row32_bf16(uint32_t tile, uint32_t r, int g, const float (&v)[32]) {
-#pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    uint4 p;
-    p.x = pack_bf16(v[8 * q + 0], v[8 * q + 1]);
-    p.y = pack_bf16(v[8 * q + 2], v[8 * q + 3]);
-    p.z = pack_bf16(v[8 * q + 4], v[8 * q + 5]);
-    p.w = pack_bf16(v[8 * q + 6], v[8 * q + 7]);
-    sts128(tile + swz(r, 4 * g + q), p);
-  }
+// ---- packed fp32x2 arithmetic (FADD2 / FMUL2 / FFMA2 on sm_100) --------------------------------
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 pk2(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ f2 pk2u(uint32_t lo, uint32_t hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi)); return r; }
+__device__ __forceinline__ void upk2(f2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ void upk2u(f2 v, uint32_t& lo, uint32_t& hi) { asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(v)); }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ uint32_t cvt_bf16x2(f2 v) {
+  float lo, hi;
+  upk2(v, lo, hi);
+  return pack_bf16(lo, hi);
+}
+
+// Address of 16-byte chunk `ch` (compile-time) of this thread's row: rowaddr = tile + (t*128 | (t&7)<<4)
+// is computed once per tile buffer; the swizzle is then one XOR with a constant.
+__device__ __forceinline__ uint32_t chunk_addr(uint32_t rowaddr, int ch) {
+  return (rowaddr ^ ((uint32_t)(ch & 7) << 4)) + (uint32_t)(ch >> 3) * kHalfBytes;
+}
+__device__ __forceinline__ void sts16(uint32_t addr, uint16_t v) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"(v) : "memory");
 }
 
 // K-major operand (rows = M or N index, K contiguous): k-step kk covers K elements 16kk..16kk+15.
@@ -110,6 +124,19 @@ __device__ __forceinline__ void issue_bx(uint32_t d_tmem, uint32_t tile_b, uint3
   umma_commit(bar);
 }
 
+// Convert 32 fp32 register values (columns 32g..32g+31 of this thread's row) to bf16 and store them.
+__device__ __forceinline__ void store_group_bf16(uint32_t rowaddr, int g, const uint32_t (&r)[32]) {
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    uint4 p;
+    p.x = pack_bf16(__uint_as_float(r[8 * q + 0]), __uint_as_float(r[8 * q + 1]));
+    p.y = pack_bf16(__uint_as_float(r[8 * q + 2]), __uint_as_float(r[8 * q + 3]));
+    p.z = pack_bf16(__uint_as_float(r[8 * q + 4]), __uint_as_float(r[8 * q + 5]));
+    p.w = pack_bf16(__uint_as_float(r[8 * q + 6]), __uint_as_float(r[8 * q + 7]));
+    sts128(chunk_addr(rowaddr, 4 * g + q), p);
+  }
+}
+
 __global__ void __launch_bounds__(kThreads, 1)
 himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __restrict__ tmaps,
                     const WorkItem* __restrict__ items, long long n_items, int mode, himuon_hparams hp, int dbg) {
@@ -126,9 +153,15 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   const uint32_t XB = smem0 + slot * kSlotBytes;
   const uint32_t AB = XB + kTileBytes;
   const uint32_t ST = AB + kTileBytes;
+  const uint32_t rowoff = (uint32_t)t * 128u + ((uint32_t)(t & 7) << 4);
+  const uint32_t xrow = XB + rowoff, arow = AB + rowoff, srow = ST + rowoff;
+  // (t, t): chunk t>>3, element t&7
+  const uint32_t diag_off = (uint32_t)(t >> 6) * kHalfBytes + (uint32_t)t * 128u +
+                            ((((uint32_t)(t >> 3) & 7u) ^ (uint32_t)(t & 7)) << 4) + (uint32_t)(t & 7) * 2u;
   SlotCtrl* sc = &ctrl->slot[slot];
   const uint32_t mma_bar = smem_u32(&sc->mma_bar);
   const uint32_t tma_bar = smem_u32(&sc->tma_bar);
+  const uint32_t dvec_addr = smem_u32(&sc->dvec[0]);
 
   if (tid == 0) {
     for (int s = 0; s < kSlots; ++s) {
@@ -143,18 +176,22 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   tc_fence_after_sync();
   const uint32_t tmem_base = ctrl->tmem_base;
   const uint32_t lane_off = (uint32_t)(wq * 32) << 16;
-  const uint32_t TX = tmem_base + slot * 256;          // fp32 X state, 128 columns
-  const uint32_t TA = TX + 128;                        // accumulator, 128 columns
+  const uint32_t TX = tmem_base + slot * 256 + lane_off;   // fp32 X state, 128 columns (this warp's lanes)
+  const uint32_t TA = TX + 128;                            // accumulator, 128 columns
+  const uint32_t TXd = tmem_base + slot * 256, TAd = TXd + 128;   // MMA destination addresses (lane 0)
   const uint32_t bar_id = 1 + slot;
 
   uint32_t ph_mma = 0, ph_tma = 0;
-  const float bc = hp.b / hp.c;
+  // The state is Xh = c^(1/4) X: then Ah = Xh Xh^T = sqrt(c) A and B = bA + cA^2 = beta Ah + Ah^2 with
+  // beta = b / sqrt(c), so the accumulator after MMA2 is B itself (no rescale in E2).
+  const float qs = sqrtf(sqrtf(hp.c));
+  const float beta_h = hp.b / sqrtf(hp.c);
 
   for (long long it = (long long)blockIdx.x * kSlots + slot; it < n_items; it += (long long)gridDim.x * kSlots) {
     WorkItem wi;
     if (items) wi = items[it];
     else { wi.layer = 0; wi.r = (int)it; wi.c = 0; wi.pad = 0; }
-    const LayerDev L = layers[wi.layer];
+    const float tau_base = layers[wi.layer].tau_base;
     const CUtensorMap* map_w = tmaps + 3 * wi.layer + 0;
     const CUtensorMap* map_g = tmaps + 3 * wi.layer + 1;
     const CUtensorMap* map_m = tmaps + 3 * wi.layer + 2;
@@ -174,17 +211,16 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     mbar_wait(tma_bar, ph_tma);
     ph_tma ^= 1;
 
-    float ss = 0.f;
-#pragma unroll 1
+    float ss = 0.f;   // this row's sum of squares of Ghat
+#pragma unroll
     for (int g = 0; g < 4; ++g) {
-      float x[32];
+      uint32_t xr[32];
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
-        const uint32_t off = swz(t, 4 * g + q);
-        const uint4 gv = lds128(AB + off);
+        const uint4 gv = lds128(chunk_addr(arow, 4 * g + q));
         const uint32_t gw[4] = {gv.x, gv.y, gv.z, gv.w};
         if (mode == MODE_STEP) {
-          const uint4 mv = lds128(ST + off);
+          const uint4 mv = lds128(chunk_addr(srow, 4 * g + q));
           const uint32_t mw[4] = {mv.x, mv.y, mv.z, mv.w};
           uint32_t mo[4];
 #pragma unroll
@@ -192,29 +228,31 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
             const float g0 = bf16_lo(gw[e]), g1 = bf16_hi(gw[e]);
             const float m0 = fmaf(hp.beta, bf16_lo(mw[e]), g0), m1 = fmaf(hp.beta, bf16_hi(mw[e]), g1);
             mo[e] = pack_bf16(m0, m1);
-            x[8 * q + 2 * e] = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;
-            x[8 * q + 2 * e + 1] = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
+            const float h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;
+            const float h1 = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
+            ss = fmaf(h0, h0, ss);
+            ss = fmaf(h1, h1, ss);
+            xr[8 * q + 2 * e] = __float_as_uint(h0);
+            xr[8 * q + 2 * e + 1] = __float_as_uint(h1);
           }
-          sts128(ST + off, make_uint4(mo[0], mo[1], mo[2], mo[3]));
+          sts128(chunk_addr(srow, 4 * g + q), make_uint4(mo[0], mo[1], mo[2], mo[3]));
         } else {
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            x[8 * q + 2 * e] = bf16_lo(gw[e]);
-            x[8 * q + 2 * e + 1] = bf16_hi(gw[e]);
+            const float h0 = bf16_lo(gw[e]), h1 = bf16_hi(gw[e]);
+            ss = fmaf(h0, h0, ss);
+            ss = fmaf(h1, h1, ss);
+            xr[8 * q + 2 * e] = __float_as_uint(h0);
+            xr[8 * q + 2 * e + 1] = __float_as_uint(h1);
           }
         }
       }
-      uint32_t xr[32];
-#pragma unroll
-      for (int j = 0; j < 32; ++j) {
-        ss = fmaf(x[j], x[j], ss);
-        xr[j] = __float_as_uint(x[j]);
-      }
-      tmem_st32(TX + lane_off + 32 * g, xr);
+      tmem_st32(TX + 32 * g, xr);
     }
+    float tot = ss;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-    if (lane == 0) sc->red[wq] = ss;
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    if (lane == 0) sc->red[wq] = tot;
     tmem_wait_st();
     fence_proxy_async_smem();          // M' in ST -> visible to the TMA store
     named_bar_sync(bar_id, kWG);
@@ -223,152 +261,139 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       tma_store_2d(map_m, x0 + 64, y0, ST + kHalfBytes);
       tma_commit_group();
     }
-    const float tot = sc->red[0] + sc->red[1] + sc->red[2] + sc->red[3];
+    tot = sc->red[0] + sc->red[1] + sc->red[2] + sc->red[3];
     const float nrm = sqrtf(tot);
-    const float inv = nrm > 0.f ? 1.f / (nrm + hp.eps) : 0.f;   // Phi_K(0) = 0
-#pragma unroll 1
-    for (int g = 0; g < 4; ++g) {
-      uint32_t xr[32];
-      tmem_ld32(TX + lane_off + 32 * g, xr);
-      tmem_wait_ld();
-      float x[32];
+    const float inv = nrm > 0.f ? qs / (nrm + hp.eps) : 0.f;   // Phi_K(0) = 0
+    float di = ss * inv * inv;                                  // diag(Ah)_t = ||Xh row t||^2 in fp32
+    {
+      const f2 inv2 = pk2(inv, inv);
 #pragma unroll
-      for (int j = 0; j < 32; ++j) {
-        x[j] = __uint_as_float(xr[j]) * inv;
-        xr[j] = __float_as_uint(x[j]);
+      for (int g = 0; g < 4; ++g) {
+        uint32_t r[32];
+        tmem_ld32(TX + 32 * g, r);
+        tmem_wait_ld();
+#pragma unroll
+        for (int j = 0; j < 16; ++j) upk2u(mul2(pk2u(r[2 * j], r[2 * j + 1]), inv2), r[2 * j], r[2 * j + 1]);
+        tmem_st32(TX + 32 * g, r);
+        store_group_bf16(xrow, g, r);
       }
-      tmem_st32(TX + lane_off + 32 * g, xr);
-      store_row32_bf16(XB, t, g, x);
     }
+    sc->dvec[t] = di;
     tmem_wait_st();
     fence_proxy_async_smem();
     tc_fence_before_sync();
     named_bar_sync(bar_id, kWG);
     if (t == 0 && hp.K > 0) {
       tc_fence_after_sync();
-      issue_gram(TA, XB, 0u, mma_bar);
+      issue_gram(TAd, XB, 0u, mma_bar);
     }
 
     uint32_t out_src = TX;   // TMEM columns the final store reads
     // ---------------- K Newton-Schulz steps ---------------------------------------------------
 #pragma unroll 1
     for (int k = 0; k < hp.K; ++k) {
-      // ---- E1: ACC = X X^T just landed
+      // ---- E1: ACC = Ah = Xh Xh^T just landed
       mbar_wait(mma_bar, ph_mma);
       ph_mma ^= 1;
       tc_fence_after_sync();
       if (dbg == 1) { out_src = TA; break; }
-      float di = 0.f;
-      {
-        uint32_t r[32];
-        tmem_ld32(TA + lane_off + 32 * wq, r);
-        tmem_wait_ld();
+      const float rowc = beta_h + di;
+      const f2 rowc2 = pk2(rowc, rowc);
+      f2 Sa = pk2(0.f, 0.f), Sb = Sa;
 #pragma unroll
-        for (int j = 0; j < 32; ++j) di = (j == lane) ? __uint_as_float(r[j]) : di;
-      }
-      sc->dvec[t] = di;
-      named_bar_sync(bar_id, kWG);
-      const float rowc = bc + di;
-#pragma unroll 1
       for (int g = 0; g < 4; ++g) {
         uint32_t r[32];
-        tmem_ld32(TA + lane_off + 32 * g, r);
+        tmem_ld32(TA + 32 * g, r);
         tmem_wait_ld();
-        float o[32];
+        store_group_bf16(arow, g, r);                      // Ob (diagonal fixed up below)
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-          const float4 dj = *reinterpret_cast<const float4*>(&sc->dvec[32 * g + 4 * q]);
-          const float dd[4] = {dj.x, dj.y, dj.z, dj.w};
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int j = 4 * q + e;
-            o[j] = __uint_as_float(r[j]);
-            r[j] = __float_as_uint(o[j] * (rowc + dd[e]));
-          }
+          const uint4 dj = lds128(dvec_addr + (32 * g + 4 * q) * 4);
+          const f2 o01 = pk2u(r[4 * q], r[4 * q + 1]), o23 = pk2u(r[4 * q + 2], r[4 * q + 3]);
+          Sa = fma2(o01, o01, Sa);
+          Sb = fma2(o23, o23, Sb);
+          upk2u(mul2(o01, add2(rowc2, pk2u(dj.x, dj.y))), r[4 * q], r[4 * q + 1]);
+          upk2u(mul2(o23, add2(rowc2, pk2u(dj.z, dj.w))), r[4 * q + 2], r[4 * q + 3]);
         }
-        if (g == wq) {
-#pragma unroll
-          for (int j = 0; j < 32; ++j)
-            if (j == lane) {
-              o[j] = 0.f;
-              r[j] = __float_as_uint(fmaf(di, di, bc * di));
-            }
-        }
-        tmem_st32(TA + lane_off + 32 * g, r);
-        store_row32_bf16(AB, t, g, o);
+        tmem_st32(TA + 32 * g, r);                          // Ah_ij (beta + d_i + d_j); diagonal unused
       }
+      sts16(AB + diag_off, 0);
+      float s0, s1;
+      upk2(add2(Sa, Sb), s0, s1);
+      const float si = hp.a + fmaf(beta_h, di, s0 + s1);    // a + B_tt, B_tt = beta d_t + (Ah^2)_tt
       tmem_wait_st();
       fence_proxy_async_smem();
       tc_fence_before_sync();
       named_bar_sync(bar_id, kWG);
       if (t == 0) {
         tc_fence_after_sync();
-        issue_gram(TA, AB, 1u, mma_bar);
+        issue_gram(TAd, AB, 1u, mma_bar);
+      }
+      // while MMA2 runs: X <- (a + B_tt) X
+      {
+        const f2 si2 = pk2(si, si);
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          uint32_t r[32];
+          tmem_ld32(TX + 32 * g, r);
+          tmem_wait_ld();
+#pragma unroll
+          for (int j = 0; j < 16; ++j) upk2u(mul2(pk2u(r[2 * j], r[2 * j + 1]), si2), r[2 * j], r[2 * j + 1]);
+          tmem_st32(TX + 32 * g, r);
+        }
+        tmem_wait_st();
       }
 
-      // ---- E2: ACC = B / c
+      // ---- E2: ACC = B (off-diagonal)
       mbar_wait(mma_bar, ph_mma);
       ph_mma ^= 1;
       tc_fence_after_sync();
       if (dbg == 2) { out_src = TA; break; }
-      float si = hp.a;
-#pragma unroll 1
+#pragma unroll
       for (int g = 0; g < 4; ++g) {
         uint32_t r[32];
-        tmem_ld32(TA + lane_off + 32 * g, r);
+        tmem_ld32(TA + 32 * g, r);
         tmem_wait_ld();
-        float o[32];
-#pragma unroll
-        for (int j = 0; j < 32; ++j) o[j] = hp.c * __uint_as_float(r[j]);
-        if (g == wq) {
-#pragma unroll
-          for (int j = 0; j < 32; ++j)
-            if (j == lane) {
-              si = hp.a + o[j];
-              o[j] = 0.f;
-            }
-        }
-        store_row32_bf16(AB, t, g, o);
+        store_group_bf16(arow, g, r);
       }
-#pragma unroll 1
-      for (int g = 0; g < 4; ++g) {
-        uint32_t r[32];
-        tmem_ld32(TX + lane_off + 32 * g, r);
-        tmem_wait_ld();
-#pragma unroll
-        for (int j = 0; j < 32; ++j) r[j] = __float_as_uint(__uint_as_float(r[j]) * si);
-        tmem_st32(TX + lane_off + 32 * g, r);
-      }
-      tmem_wait_st();
+      sts16(AB + diag_off, 0);
       fence_proxy_async_smem();
       tc_fence_before_sync();
       named_bar_sync(bar_id, kWG);
       if (t == 0) {
         tc_fence_after_sync();
-        issue_bx(TX, AB, XB, mma_bar);
+        issue_bx(TXd, AB, XB, mma_bar);
       }
 
-      // ---- E3: X = aX + BX
+      // ---- E3: Xh = (a + B_tt) Xh + offdiag(B) Xh
       mbar_wait(mma_bar, ph_mma);
       ph_mma ^= 1;
       tc_fence_after_sync();
       if (k + 1 < hp.K) {
-#pragma unroll 1
+        f2 Da = pk2(0.f, 0.f), Db = Da;
+#pragma unroll
         for (int g = 0; g < 4; ++g) {
           uint32_t r[32];
-          tmem_ld32(TX + lane_off + 32 * g, r);
+          tmem_ld32(TX + 32 * g, r);
           tmem_wait_ld();
-          float x[32];
+          store_group_bf16(xrow, g, r);
 #pragma unroll
-          for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
-          store_row32_bf16(XB, t, g, x);
+          for (int j = 0; j < 8; ++j) {
+            const f2 x01 = pk2u(r[4 * j], r[4 * j + 1]), x23 = pk2u(r[4 * j + 2], r[4 * j + 3]);
+            Da = fma2(x01, x01, Da);
+            Db = fma2(x23, x23, Db);
+          }
         }
+        float d0, d1;
+        upk2(add2(Da, Db), d0, d1);
+        di = d0 + d1;
+        sc->dvec[t] = di;
         fence_proxy_async_smem();
         tc_fence_before_sync();
         named_bar_sync(bar_id, kWG);
         if (t == 0) {
           tc_fence_after_sync();
-          issue_gram(TA, XB, 0u, mma_bar);
+          issue_gram(TAd, XB, 0u, mma_bar);
         }
       }
     }
@@ -388,40 +413,36 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       named_bar_sync(bar_id, kWG);
     }
     const float keep = 1.f - hp.lr * hp.wd;
-    const float stepsz = hp.lr * hp.scale_c * L.tau_base;
-#pragma unroll 1
+    const float unq = dbg ? 1.f : 1.f / qs;                       // undo the c^(1/4) state scaling
+    const float stepsz = -hp.lr * hp.scale_c * tau_base * unq;
+#pragma unroll
     for (int g = 0; g < 4; ++g) {
       uint32_t r[32];
-      tmem_ld32(out_src + lane_off + 32 * g, r);
+      tmem_ld32(out_src + 32 * g, r);
       tmem_wait_ld();
-      float x[32];
-#pragma unroll
-      for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
       if (mode == MODE_STEP) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          const uint4 wv = lds128(ST + swz(t, 4 * g + q));
+          const uint4 wv = lds128(chunk_addr(srow, 4 * g + q));
           const uint32_t ww[4] = {wv.x, wv.y, wv.z, wv.w};
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            x[8 * q + 2 * e] = fmaf(keep, bf16_lo(ww[e]), -stepsz * x[8 * q + 2 * e]);
-            x[8 * q + 2 * e + 1] = fmaf(keep, bf16_hi(ww[e]), -stepsz * x[8 * q + 2 * e + 1]);
+            r[8 * q + 2 * e] = __float_as_uint(fmaf(keep, bf16_lo(ww[e]), stepsz * __uint_as_float(r[8 * q + 2 * e])));
+            r[8 * q + 2 * e + 1] = __float_as_uint(fmaf(keep, bf16_hi(ww[e]), stepsz * __uint_as_float(r[8 * q + 2 * e + 1])));
           }
         }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 32; ++j) r[j] = __float_as_uint(__uint_as_float(r[j]) * unq);
       }
-      store_row32_bf16(ST, t, g, x);
+      store_group_bf16(srow, g, r);
     }
     fence_proxy_async_smem();
-    tc_fence_before_sync();
     named_bar_sync(bar_id, kWG);
     if (t == 0) {
       tma_store_2d(map_w, x0, y0, ST);
       tma_store_2d(map_w, x0 + 64, y0, ST + kHalfBytes);
       tma_commit_group();
-    }
-    if (dbg != 0 && hp.K > 0) {
-      // debug early-out left an MMA chain unfinished only if we broke before issuing the next one:
-      // nothing pending here (every issued batch was waited on), so the slot is clean.
     }
   }
 

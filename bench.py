@@ -199,6 +199,7 @@ def run_gpu(args):
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    torch.cuda.profiler.start()       # no-op unless run under `ncu --profile-from-start off`
     t_begin.record(stream)
     for k in range(args.steps):
         evs[k][0].record(stream)
@@ -206,6 +207,7 @@ def run_gpu(args):
         evs[k][1].record(stream)
     t_end.record(stream)
     barrier()
+    torch.cuda.profiler.stop()
     launches = hm.himuon_launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
     total_ms = t_begin.elapsed_time(t_end)

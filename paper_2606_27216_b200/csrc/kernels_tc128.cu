@@ -1,24 +1,33 @@
 // Tensor-core path of the HiMuon hot path for T = 128, bf16 storage (sm_100a: TMA + tcgen05 + TMEM).
 //
-// One persistent CTA per SM holds TWO tiles in flight ("slots"); each slot is served by its own
-// warpgroup (thread t of the warpgroup <-> row t of the tile <-> TMEM lane t).  While one slot's
-// warpgroup runs an epilogue on CUDA cores, the other slot's MMAs run on the tensor pipe.
+// One persistent CTA per SM holds TWO tiles in flight ("slots").  A slot is served by 8 warps:
+// thread (t, h) owns row t of the tile (= TMEM lane t) and the column half h (columns 64h..64h+63).
+// While one slot's warps run an epilogue on the CUDA cores, the other slot's MMAs run on the tensor
+// pipe.  What the profile of the previous version showed (profiles/r1_tc128_v2_ncu_full.md) shaped
+// this one: an SS-mode 128x128x16 MMA reads 8 KB of operands per 64 cycles, i.e. the whole
+// shared-memory data path, and the epilogues' own smem traffic competes with it.  Here
+//   * the A operand of every MMA lives in tensor memory (tcgen05.mma with A in TMEM), so an MMA
+//     takes half the smem bandwidth and B_b (the A operand of MMA3) never touches smem;
+//   * the fp32 iterate X lives in REGISTERS (64 per thread), which frees TMEM for the operand and
+//     removes the separate "X <- (a + B_tt) X" pass over tensor memory;
+//   * the next tile's G and M and this tile's W are fetched by TMA while the NS steps run.
 //
 // Per tile (Alg. 4.1; Eq. 2.2-2.3; Eq. 4.6), everything between the TMA loads of
 // G, M, W and the TMA stores of M, W stays on chip:
-//   P   TMA G,M -> smem; M' = beta M + G; Ghat = G + beta M' (Nesterov) | M'; M' -> TMA store;
-//       Xh0 = q Ghat / (||Ghat||_F + eps), q = c^(1/4)  -> fp32 in TMEM (state), bf16 in smem (operand)
+//   P   G, M (smem) -> M' = beta M + G; Ghat = G + beta M' (Nesterov) | M'; M' -> TMA store;
+//       Xh0 = q Ghat / (||Ghat||_F + eps), q = c^(1/4): fp32 in registers (state),
+//       bf16 in smem XB (B operand) and in TMEM OPA (A operand)
 //       (with the state scaled by q: Ah = Xh Xh^T = sqrt(c) A and B = bA + cA^2 = beta Ah + Ah^2,
 //        beta = b / sqrt(c), so no accumulator ever needs a rescale by c)
 //   K x MMA1  ACC  = Xb Xb^T                                   (Ah)
-//       E1    Ob = bf16(ACC), diagonal zeroed -> smem;  S_t = sum_j ACC_tj^2 = (Ah^2)_tt  (fp32)
-//             ACC <- ACC_ij (beta + d_i + d_j),  d_t = ||Xh row t||^2 = (Ah)_tt  (fp32)
-//       MMA2  ACC += Ob Ob^T                                   (=> ACC_ij = B_ij for i != j)
-//             meanwhile: X <- (a + B_tt) X,  B_tt = beta d_t + S_t          (fp32, TMEM, row scaling)
-//       E2    bf16(ACC), diagonal zeroed -> smem
-//       MMA3  X += offdiag(B)b Xb                              (=> Xh = a Xh + B Xh)
-//       E3    Xb = bf16(X) -> smem;  d_t = sum_j X_tj^2
-//   F   TMA W -> smem; W' = (1 - lr wd) W - lr tau X_K / q -> TMA store   (Phi mode: store X_K / q)
+//       E1    Ot = bf16(offdiag(ACC) + diag(d + beta/2)) -> smem OB + TMEM OPA,  d_t = ||Xh row t||^2 (fp32);
+//             S_t = sum_j ACC_tj^2 = (Ah^2)_tt  (fp32)
+//       MMA2  ACC  = Ot Ot^T      (=> ACC_ij = (O^2)_ij + (beta + d_i + d_j) O_ij = B_ij for i != j)
+//       E2    Bb = bf16(ACC), diagonal zeroed -> TMEM OPA
+//       MMA3  ACC  = Bb Xb                                     (offdiag(B) Xh)
+//       E3    X <- (a + B_tt) X + ACC, B_tt = beta d_t + S_t (fp32 row scaling, registers);
+//             Xb = bf16(X) -> smem XB + TMEM OPA;  d_t = sum_j X_tj^2
+//   F   W (smem, prefetched) ; W' = (1 - lr wd) W - lr tau X_K / q -> TMA store (Phi mode: X_K / q)
 // The diagonals of A and B (O(1) numbers whose bf16 rounding would dominate the error) never pass
 // through bf16: they act as fp32 row scalings.  DESIGN.md "Numerical scheme" derives the algebra.
 //
@@ -26,6 +35,7 @@
 // PAPER.md:51-53) and the TMA stores clip (= the crop of B_T^-1); padded rows and
 // columns stay exactly zero through Eq. 2.2.
 #include <cuda_bf16.h>
+#include <stddef.h>
 
 #include "himuon_internal.h"
 #include "sm100_ptx.cuh"
@@ -40,32 +50,29 @@ using namespace ptx;
 
 constexpr int T = 128;
 constexpr int kSlots = 2;
-constexpr int kWG = 128;                         // threads per slot
-constexpr int kThreads = kSlots * kWG;
+constexpr int kSlotThreads = 256;                // 8 warps: 4 lane quadrants x 2 column halves
+constexpr int kThreads = kSlots * kSlotThreads;
 constexpr uint32_t kTileBytes = T * T * 2;       // 32 KB: one bf16 tile
 constexpr uint32_t kHalfBytes = kTileBytes / 2;  // one 64-column block (128 rows x 128 B)
-constexpr uint32_t kSlotBytes = 3 * kTileBytes;  // XB, AB, ST
-constexpr uint32_t kCtrlBytes = 2048;
+constexpr uint32_t kSlotBytes = 3 * kTileBytes;  // XB, OB, ST
+constexpr uint32_t kCtrlBytes = 8192;
 constexpr uint32_t kSmemBytes = kSlots * kSlotBytes + kCtrlBytes + 1024;  // + alignment slack
+constexpr uint32_t kSlotCols = 256;              // TMEM columns per slot: ACC 128 (fp32) + OPA 64 (bf16 pairs)
+constexpr uint32_t kOpaCol = 128;
 
 struct SlotCtrl {
-  unsigned long long mma_bar;
-  unsigned long long tma_bar;
-  float dvec[T];
-  float red[4];
+  unsigned long long mma_bar;   // tcgen05.commit of MMA1 / MMA2 / MMA3
+  unsigned long long ld_bar;    // TMA loads of G (and M) of the next tile
+  unsigned long long w_bar;     // TMA load of W
+  float dpart[2][T];            // per column half: partial d_t = sum_j Xh_tj^2
+  float spart[2][T];            // per column half: sum_j ACC_tj^2
+  float red[8];
 };
 struct Ctrl {
   SlotCtrl slot[kSlots];
   uint32_t tmem_base;
 };
 static_assert(sizeof(Ctrl) <= kCtrlBytes, "control block too large");
-
-// byte offset of 16-byte chunk `ch` (0..15) of row `r` in a [128 x 128] bf16 tile stored as two
-// 64-column blocks in the 128-byte-swizzled K-major layout (what TMA SWIZZLE_128B writes and what
-// the UMMA descriptors below read).
-__device__ __forceinline__ uint32_t swz(uint32_t r, uint32_t ch) {
-  return (ch >> 3) * kHalfBytes + r * 128u + (((ch & 7u) ^ (r & 7u)) << 4);
-}
 
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
@@ -89,14 +96,10 @@ __device__ __forceinline__ uint32_t cvt_bf16x2(f2 v) {
   return pack_bf16(lo, hi);
 }
 
-// Address of 16-byte chunk `ch` (compile-time) of this thread's row: rowaddr = tile + (t*128 | (t&7)<<4)
-// is computed once per tile buffer; the swizzle is then one XOR with a constant.
-__device__ __forceinline__ uint32_t chunk_addr(uint32_t rowaddr, int ch) {
-  return (rowaddr ^ ((uint32_t)(ch & 7) << 4)) + (uint32_t)(ch >> 3) * kHalfBytes;
-}
-__device__ __forceinline__ void sts16(uint32_t addr, uint16_t v) {
-  asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"(v) : "memory");
-}
+// A [128 x 128] bf16 tile is stored as two 64-column blocks in the 128-byte-swizzled K-major layout
+// (what TMA SWIZZLE_128B writes and what the UMMA descriptors below read).  `rowaddr` =
+// block(h) + t*128 + ((t&7)<<4); 16-byte chunk c (0..7) of this thread's 64 columns is then one XOR away.
+__device__ __forceinline__ uint32_t chunk_addr(uint32_t rowaddr, int c) { return rowaddr ^ ((uint32_t)c << 4); }
 
 // K-major operand (rows = M or N index, K contiguous): k-step kk covers K elements 16kk..16kk+15.
 __device__ __forceinline__ uint64_t desc_kmajor(uint32_t tile, int kk) {
@@ -108,33 +111,30 @@ __device__ __forceinline__ uint64_t desc_mnmajor(uint32_t tile, int kk) {
   return make_smem_desc_sw128(tile + kk * 2048, kHalfBytes, 1024);
 }
 
-__device__ __forceinline__ void issue_gram(uint32_t d_tmem, uint32_t tile, uint32_t accumulate, uint32_t bar) {
+// ACC (+)= OPA * tile^T  (A = bf16 [128 x 128] in TMEM, B = K-major smem tile)
+__device__ __forceinline__ void issue_gram(uint32_t acc, uint32_t opa, uint32_t tile, uint32_t accumulate, uint32_t bar) {
   constexpr uint32_t idesc = make_idesc_bf16(T, T, 0, 0);
 #pragma unroll
-  for (int kk = 0; kk < T / 16; ++kk) {
-    const uint64_t d = desc_kmajor(tile, kk);
-    umma_bf16_ss(d_tmem, d, d, idesc, (accumulate | (uint32_t)kk) ? 1u : 0u);
-  }
+  for (int kk = 0; kk < T / 16; ++kk)
+    umma_bf16_ts(acc, opa + 8 * kk, desc_kmajor(tile, kk), idesc, (accumulate | (uint32_t)kk) ? 1u : 0u);
   umma_commit(bar);
 }
-__device__ __forceinline__ void issue_bx(uint32_t d_tmem, uint32_t tile_b, uint32_t tile_x, uint32_t bar) {
+// ACC = OPA * tile  (A = bf16 [128 x 128] in TMEM, B = the K-major tile read MN-major, i.e. not transposed)
+__device__ __forceinline__ void issue_bx(uint32_t acc, uint32_t opa, uint32_t tile_x, uint32_t bar) {
   constexpr uint32_t idesc = make_idesc_bf16(T, T, 0, 1);
 #pragma unroll
-  for (int kk = 0; kk < T / 16; ++kk) umma_bf16_ss(d_tmem, desc_kmajor(tile_b, kk), desc_mnmajor(tile_x, kk), idesc, 1u);
+  for (int kk = 0; kk < T / 16; ++kk) umma_bf16_ts(acc, opa + 8 * kk, desc_mnmajor(tile_x, kk), idesc, kk ? 1u : 0u);
   umma_commit(bar);
 }
 
-// Convert 32 fp32 register values (columns 32g..32g+31 of this thread's row) to bf16 and store them.
-__device__ __forceinline__ void store_group_bf16(uint32_t rowaddr, int g, const uint32_t (&r)[32]) {
+// Replace one bf16 of a packed 16-column chunk: word `idx` (0..7, or 8 for none) becomes (word & keep) | val.
+__device__ __forceinline__ void set_one(uint32_t (&p)[8], int idx, uint32_t keep, uint32_t val) {
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    uint4 p;
-    p.x = pack_bf16(__uint_as_float(r[8 * q + 0]), __uint_as_float(r[8 * q + 1]));
-    p.y = pack_bf16(__uint_as_float(r[8 * q + 2]), __uint_as_float(r[8 * q + 3]));
-    p.z = pack_bf16(__uint_as_float(r[8 * q + 4]), __uint_as_float(r[8 * q + 5]));
-    p.w = pack_bf16(__uint_as_float(r[8 * q + 6]), __uint_as_float(r[8 * q + 7]));
-    sts128(chunk_addr(rowaddr, 4 * g + q), p);
-  }
+  for (int j = 0; j < 8; ++j) p[j] = (j == idx) ? ((p[j] & keep) | val) : p[j];
+}
+__device__ __forceinline__ void pack16(const uint32_t (&r)[16], uint32_t (&p)[8]) {
+#pragma unroll
+  for (int j = 0; j < 8; ++j) p[j] = pack_bf16(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -145,28 +145,31 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   Ctrl* ctrl = reinterpret_cast<Ctrl*>(smem_raw + (smem0 - smem_u32(smem_raw)) + kSlots * kSlotBytes);
 
   const int tid = threadIdx.x;
-  const int slot = tid / kWG;
-  const int t = tid % kWG;            // row of the tile / TMEM lane
-  const int wq = (tid >> 5) & 3;      // TMEM lane quadrant of this warp
+  const int slot = tid / kSlotThreads;
+  const int ts = tid % kSlotThreads;
+  const int w = ts >> 5;               // warp of the slot
+  const int wq = w & 3;                // TMEM lane quadrant of this warp (= warp index in the CTA mod 4)
+  const int h = w >> 2;                // column half
   const int lane = tid & 31;
+  const int t = wq * 32 + lane;        // row of the tile / TMEM lane
+  const bool lead = (ts == 0);
+  const bool step_mode = (mode == MODE_STEP);
 
   const uint32_t XB = smem0 + slot * kSlotBytes;
-  const uint32_t AB = XB + kTileBytes;
-  const uint32_t ST = AB + kTileBytes;
-  const uint32_t rowoff = (uint32_t)t * 128u + ((uint32_t)(t & 7) << 4);
-  const uint32_t xrow = XB + rowoff, arow = AB + rowoff, srow = ST + rowoff;
-  // (t, t): chunk t>>3, element t&7
-  const uint32_t diag_off = (uint32_t)(t >> 6) * kHalfBytes + (uint32_t)t * 128u +
-                            ((((uint32_t)(t >> 3) & 7u) ^ (uint32_t)(t & 7)) << 4) + (uint32_t)(t & 7) * 2u;
+  const uint32_t OB = XB + kTileBytes;
+  const uint32_t ST = OB + kTileBytes;
+  const uint32_t rowoff = (uint32_t)h * kHalfBytes + (uint32_t)t * 128u + ((uint32_t)(t & 7) << 4);
+  const uint32_t xrow = XB + rowoff, orow = OB + rowoff, srow = ST + rowoff;
   SlotCtrl* sc = &ctrl->slot[slot];
   const uint32_t mma_bar = smem_u32(&sc->mma_bar);
-  const uint32_t tma_bar = smem_u32(&sc->tma_bar);
-  const uint32_t dvec_addr = smem_u32(&sc->dvec[0]);
+  const uint32_t ld_bar = smem_u32(&sc->ld_bar);
+  const uint32_t w_bar = smem_u32(&sc->w_bar);
 
   if (tid == 0) {
     for (int s = 0; s < kSlots; ++s) {
       mbar_init(smem_u32(&ctrl->slot[s].mma_bar), 1);
-      mbar_init(smem_u32(&ctrl->slot[s].tma_bar), 1);
+      mbar_init(smem_u32(&ctrl->slot[s].ld_bar), 2);   // arrive.expect_tx at issue + "staging is free" arrive
+      mbar_init(smem_u32(&ctrl->slot[s].w_bar), 1);
     }
     fence_mbar_init();
   }
@@ -174,282 +177,343 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   tc_fence_before_sync();
   __syncthreads();
   tc_fence_after_sync();
-  const uint32_t tmem_base = ctrl->tmem_base;
+  const uint32_t tmem_slot = ctrl->tmem_base + slot * kSlotCols;        // lane 0: MMA operand / destination addresses
   const uint32_t lane_off = (uint32_t)(wq * 32) << 16;
-  const uint32_t TX = tmem_base + slot * 256 + lane_off;   // fp32 X state, 128 columns (this warp's lanes)
-  const uint32_t TA = TX + 128;                            // accumulator, 128 columns
-  const uint32_t TXd = tmem_base + slot * 256, TAd = TXd + 128;   // MMA destination addresses (lane 0)
+  const uint32_t acc_t = tmem_slot + lane_off + 64u * h;                 // this thread's 64 accumulator columns
+  const uint32_t opa_t = tmem_slot + lane_off + kOpaCol + 32u * h;       // this thread's 32 packed operand columns
+  const uint32_t ACCd = tmem_slot, OPAd = tmem_slot + kOpaCol;
   const uint32_t bar_id = 1 + slot;
 
-  uint32_t ph_mma = 0, ph_tma = 0;
+  uint32_t ph_mma = 0, ph_ld = 0, ph_w = 0;
   // The state is Xh = c^(1/4) X: then Ah = Xh Xh^T = sqrt(c) A and B = bA + cA^2 = beta Ah + Ah^2 with
   // beta = b / sqrt(c), so the accumulator after MMA2 is B itself (no rescale in E2).
   const float qs = sqrtf(sqrtf(hp.c));
   const float beta_h = hp.b / sqrtf(hp.c);
+  const long long stride = (long long)gridDim.x * kSlots;
 
-  for (long long it = (long long)blockIdx.x * kSlots + slot; it < n_items; it += (long long)gridDim.x * kSlots) {
+  // ---- TMA issue helpers (lead thread of the slot only) ----------------------------------------------
+  auto item_at = [&](long long i) {
     WorkItem wi;
-    if (items) wi = items[it];
-    else { wi.layer = 0; wi.r = (int)it; wi.c = 0; wi.pad = 0; }
+    if (items) wi = items[i];
+    else { wi.layer = 0; wi.r = (int)i; wi.c = 0; wi.pad = 0; }
+    return wi;
+  };
+  auto issue_g = [&](long long i) {      // G of tile i -> OB; arms ld_bar for G and (step mode) M
+    const WorkItem wi = item_at(i);
+    const CUtensorMap* map_g = tmaps + 3 * wi.layer + 1;
+    mbar_arrive_expect_tx(ld_bar, step_mode ? 2 * kTileBytes : kTileBytes);
+    tma_load_2d(OB, map_g, wi.c * T, wi.r * T, ld_bar);
+    tma_load_2d(OB + kHalfBytes, map_g, wi.c * T + 64, wi.r * T, ld_bar);
+  };
+  auto issue_m = [&](long long i) {      // M of tile i -> XB
+    const WorkItem wi = item_at(i);
+    const CUtensorMap* map_m = tmaps + 3 * wi.layer + 2;
+    tma_load_2d(XB, map_m, wi.c * T, wi.r * T, ld_bar);
+    tma_load_2d(XB + kHalfBytes, map_m, wi.c * T + 64, wi.r * T, ld_bar);
+  };
+
+  long long it = (long long)blockIdx.x * kSlots + slot;
+  if (lead && it < n_items) {
+    issue_g(it);
+    if (step_mode) issue_m(it);
+  }
+
+  for (; it < n_items; it += stride) {
+    const WorkItem wi = item_at(it);
     const float tau_base = layers[wi.layer].tau_base;
     const CUtensorMap* map_w = tmaps + 3 * wi.layer + 0;
-    const CUtensorMap* map_g = tmaps + 3 * wi.layer + 1;
     const CUtensorMap* map_m = tmaps + 3 * wi.layer + 2;
     const int x0 = wi.c * T, y0 = wi.r * T;
+    const long long nxt = it + stride;
+    bool g_issued = false, m_issued = false, w_issued = false;   // meaningful in the lead thread only
+    // the diagonal element (t, t): 16-column chunk t>>4 of the row, packed word (t&15)>>1, half t&1
+    const int dchunk = t >> 4, dword = (t & 15) >> 1;
+    const uint32_t dkeep = (t & 1) ? 0x0000ffffu : 0xffff0000u;
 
-    // ---------------- P: load, momentum, normalise -------------------------------------------
-    if (t == 0) {
+    // ---------------- P: momentum, normalise ---------------------------------------------------
+    if (lead) {
       tma_wait_group_read0();   // the previous tile's stores out of ST have been read
-      mbar_arrive_expect_tx(tma_bar, mode == MODE_STEP ? 2 * kTileBytes : kTileBytes);
-      tma_load_2d(AB, map_g, x0, y0, tma_bar);
-      tma_load_2d(AB + kHalfBytes, map_g, x0 + 64, y0, tma_bar);
-      if (mode == MODE_STEP) {
-        tma_load_2d(ST, map_m, x0, y0, tma_bar);
-        tma_load_2d(ST + kHalfBytes, map_m, x0 + 64, y0, tma_bar);
-      }
+      mbar_arrive(ld_bar);
     }
-    mbar_wait(tma_bar, ph_tma);
-    ph_tma ^= 1;
+    mbar_wait(ld_bar, ph_ld);
+    ph_ld ^= 1;
 
-    float ss = 0.f;   // this row's sum of squares of Ghat
+    f2 xs[32];                  // fp32 state: this thread's 64 columns of row t, as packed pairs
+    float ss = 0.f;             // sum of squares of this thread's part of Ghat
 #pragma unroll
-    for (int g = 0; g < 4; ++g) {
-      uint32_t xr[32];
+    for (int c = 0; c < 8; ++c) {
+      const uint4 gv = lds128(chunk_addr(orow, c));
+      const uint32_t gw[4] = {gv.x, gv.y, gv.z, gv.w};
+      if (step_mode) {
+        const uint4 mv = lds128(chunk_addr(xrow, c));
+        const uint32_t mw[4] = {mv.x, mv.y, mv.z, mv.w};
+        uint32_t mo[4];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const uint4 gv = lds128(chunk_addr(arow, 4 * g + q));
-        const uint32_t gw[4] = {gv.x, gv.y, gv.z, gv.w};
-        if (mode == MODE_STEP) {
-          const uint4 mv = lds128(chunk_addr(srow, 4 * g + q));
-          const uint32_t mw[4] = {mv.x, mv.y, mv.z, mv.w};
-          uint32_t mo[4];
+        for (int e = 0; e < 4; ++e) {
+          const float g0 = bf16_lo(gw[e]), g1 = bf16_hi(gw[e]);
+          const float m0 = fmaf(hp.beta, bf16_lo(mw[e]), g0), m1 = fmaf(hp.beta, bf16_hi(mw[e]), g1);
+          mo[e] = pack_bf16(m0, m1);
+          const float h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;
+          const float h1 = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
+          ss = fmaf(h0, h0, ss);
+          ss = fmaf(h1, h1, ss);
+          xs[4 * c + e] = pk2(h0, h1);
+        }
+        sts128(chunk_addr(srow, c), make_uint4(mo[0], mo[1], mo[2], mo[3]));
+      } else {
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float g0 = bf16_lo(gw[e]), g1 = bf16_hi(gw[e]);
-            const float m0 = fmaf(hp.beta, bf16_lo(mw[e]), g0), m1 = fmaf(hp.beta, bf16_hi(mw[e]), g1);
-            mo[e] = pack_bf16(m0, m1);
-            const float h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;
-            const float h1 = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
-            ss = fmaf(h0, h0, ss);
-            ss = fmaf(h1, h1, ss);
-            xr[8 * q + 2 * e] = __float_as_uint(h0);
-            xr[8 * q + 2 * e + 1] = __float_as_uint(h1);
-          }
-          sts128(chunk_addr(srow, 4 * g + q), make_uint4(mo[0], mo[1], mo[2], mo[3]));
-        } else {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float h0 = bf16_lo(gw[e]), h1 = bf16_hi(gw[e]);
-            ss = fmaf(h0, h0, ss);
-            ss = fmaf(h1, h1, ss);
-            xr[8 * q + 2 * e] = __float_as_uint(h0);
-            xr[8 * q + 2 * e + 1] = __float_as_uint(h1);
-          }
+        for (int e = 0; e < 4; ++e) {
+          const float h0 = bf16_lo(gw[e]), h1 = bf16_hi(gw[e]);
+          ss = fmaf(h0, h0, ss);
+          ss = fmaf(h1, h1, ss);
+          xs[4 * c + e] = pk2(h0, h1);
         }
       }
-      tmem_st32(TX + 32 * g, xr);
     }
     float tot = ss;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-    if (lane == 0) sc->red[wq] = tot;
-    tmem_wait_st();
+    if (lane == 0) sc->red[w] = tot;
     fence_proxy_async_smem();          // M' in ST -> visible to the TMA store
-    named_bar_sync(bar_id, kWG);
-    if (t == 0 && mode == MODE_STEP) {
+    named_bar_sync(bar_id, kSlotThreads);
+    if (lead && step_mode) {
       tma_store_2d(map_m, x0, y0, ST);
       tma_store_2d(map_m, x0 + 64, y0, ST + kHalfBytes);
       tma_commit_group();
     }
-    tot = sc->red[0] + sc->red[1] + sc->red[2] + sc->red[3];
+    tot = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) tot += sc->red[i];
     const float nrm = sqrtf(tot);
     const float inv = nrm > 0.f ? qs / (nrm + hp.eps) : 0.f;   // Phi_K(0) = 0
-    float di = ss * inv * inv;                                  // diag(Ah)_t = ||Xh row t||^2 in fp32
+    sc->dpart[h][t] = ss * inv * inv;                           // partial diag(Ah)_t in fp32
     {
       const f2 inv2 = pk2(inv, inv);
 #pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        uint32_t r[32];
-        tmem_ld32(TX + 32 * g, r);
-        tmem_wait_ld();
+      for (int q = 0; q < 4; ++q) {
+        uint32_t p[8];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) upk2u(mul2(pk2u(r[2 * j], r[2 * j + 1]), inv2), r[2 * j], r[2 * j + 1]);
-        tmem_st32(TX + 32 * g, r);
-        store_group_bf16(xrow, g, r);
+        for (int j = 0; j < 8; ++j) {
+          xs[8 * q + j] = mul2(xs[8 * q + j], inv2);
+          p[j] = cvt_bf16x2(xs[8 * q + j]);
+        }
+        sts128(chunk_addr(xrow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
+        sts128(chunk_addr(xrow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
+        tmem_st8(opa_t + 8 * q, p);
       }
     }
-    sc->dvec[t] = di;
     tmem_wait_st();
     fence_proxy_async_smem();
     tc_fence_before_sync();
-    named_bar_sync(bar_id, kWG);
-    if (t == 0 && hp.K > 0) {
+    named_bar_sync(bar_id, kSlotThreads);
+    if (lead && hp.K > 0) {
       tc_fence_after_sync();
-      issue_gram(TAd, XB, 0u, mma_bar);
+      issue_gram(ACCd, OPAd, XB, 0u, mma_bar);
     }
+    float di = sc->dpart[0][t] + sc->dpart[1][t];   // d_t = (Ah)_tt in fp32, from the fp32 state
 
-    uint32_t out_src = TX;   // TMEM columns the final store reads
+    bool dumped = false;   // debug stages: xs holds a raw accumulator dump instead of X_K
     // ---------------- K Newton-Schulz steps ---------------------------------------------------
 #pragma unroll 1
     for (int k = 0; k < hp.K; ++k) {
+      const bool last = (k + 1 == hp.K);
       // ---- E1: ACC = Ah = Xh Xh^T just landed
       mbar_wait(mma_bar, ph_mma);
       ph_mma ^= 1;
       tc_fence_after_sync();
-      if (dbg == 1) { out_src = TA; break; }
-      const float rowc = beta_h + di;
-      const f2 rowc2 = pk2(rowc, rowc);
-      f2 Sa = pk2(0.f, 0.f), Sb = Sa;
+      if (dbg == 1) { dumped = true; break; }
+      {
+        // Ot = offdiag(Ah) + diag(d + beta/2), rounded to bf16: then for i != j
+        //   (Ot Ot^T)_ij = (O^2)_ij + (beta + d_i + d_j) O_ij = (beta Ah + Ah^2)_ij = B_ij.
+        const uint32_t dval = (pack_bf16(fmaf(0.5f, beta_h, di), 0.f) & 0xffffu) << ((t & 1) * 16);
+        f2 Sa = pk2(0.f, 0.f), Sb = Sa;
+        uint32_t r[2][16];
+        tmem_ld16(acc_t, r[0]);
 #pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        uint32_t r[32];
-        tmem_ld32(TA + 32 * g, r);
-        tmem_wait_ld();
-        store_group_bf16(arow, g, r);                      // Ob (diagonal fixed up below)
+        for (int q = 0; q < 4; ++q) {
+          tmem_wait_ld();
+          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          uint32_t(&c)[16] = r[q & 1];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
-          const uint4 dj = lds128(dvec_addr + (32 * g + 4 * q) * 4);
-          const f2 o01 = pk2u(r[4 * q], r[4 * q + 1]), o23 = pk2u(r[4 * q + 2], r[4 * q + 3]);
-          Sa = fma2(o01, o01, Sa);
-          Sb = fma2(o23, o23, Sb);
-          upk2u(mul2(o01, add2(rowc2, pk2u(dj.x, dj.y))), r[4 * q], r[4 * q + 1]);
-          upk2u(mul2(o23, add2(rowc2, pk2u(dj.z, dj.w))), r[4 * q + 2], r[4 * q + 3]);
+          for (int j = 0; j < 4; ++j) {
+            const f2 o01 = pk2u(c[4 * j], c[4 * j + 1]), o23 = pk2u(c[4 * j + 2], c[4 * j + 3]);
+            Sa = fma2(o01, o01, Sa);
+            Sb = fma2(o23, o23, Sb);
+          }
+          uint32_t p[8];
+          pack16(c, p);
+          // warp-uniform test: this chunk pair holds the diagonal of the warp's rows
+          if ((((h << 2) + q) >> 1) == wq) set_one(p, dchunk == (h << 2) + q ? dword : 8, dkeep, dval);
+          sts128(chunk_addr(orow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
+          sts128(chunk_addr(orow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
+          tmem_st8(opa_t + 8 * q, p);
         }
-        tmem_st32(TA + 32 * g, r);                          // Ah_ij (beta + d_i + d_j); diagonal unused
+        float s0, s1;
+        upk2(add2(Sa, Sb), s0, s1);
+        sc->spart[h][t] = s0 + s1;
       }
-      sts16(AB + diag_off, 0);
-      float s0, s1;
-      upk2(add2(Sa, Sb), s0, s1);
-      const float si = hp.a + fmaf(beta_h, di, s0 + s1);    // a + B_tt, B_tt = beta d_t + (Ah^2)_tt
+      if (lead && step_mode && !w_issued) {                 // M' has left ST by now: fetch W into it
+        tma_wait_group_read0();
+        mbar_arrive_expect_tx(w_bar, kTileBytes);
+        tma_load_2d(ST, map_w, x0, y0, w_bar);
+        tma_load_2d(ST + kHalfBytes, map_w, x0 + 64, y0, w_bar);
+        w_issued = true;
+      }
       tmem_wait_st();
       fence_proxy_async_smem();
       tc_fence_before_sync();
-      named_bar_sync(bar_id, kWG);
-      if (t == 0) {
+      named_bar_sync(bar_id, kSlotThreads);
+      if (lead) {
         tc_fence_after_sync();
-        issue_gram(TAd, AB, 1u, mma_bar);
+        issue_gram(ACCd, OPAd, OB, 0u, mma_bar);
       }
-      // while MMA2 runs: X <- (a + B_tt) X
-      {
-        const f2 si2 = pk2(si, si);
-#pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          uint32_t r[32];
-          tmem_ld32(TX + 32 * g, r);
-          tmem_wait_ld();
-#pragma unroll
-          for (int j = 0; j < 16; ++j) upk2u(mul2(pk2u(r[2 * j], r[2 * j + 1]), si2), r[2 * j], r[2 * j + 1]);
-          tmem_st32(TX + 32 * g, r);
-        }
-        tmem_wait_st();
-      }
+      // a + B_tt, B_tt = beta d_t + (Ah^2)_tt
+      const float si = hp.a + fmaf(beta_h, di, sc->spart[0][t] + sc->spart[1][t]);
 
       // ---- E2: ACC = B (off-diagonal)
       mbar_wait(mma_bar, ph_mma);
       ph_mma ^= 1;
       tc_fence_after_sync();
-      if (dbg == 2) { out_src = TA; break; }
-#pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        uint32_t r[32];
-        tmem_ld32(TA + 32 * g, r);
-        tmem_wait_ld();
-        store_group_bf16(arow, g, r);
+      if (dbg == 2) { dumped = true; break; }
+      if (lead && last && nxt < n_items) {                  // OB is free: fetch the next tile's G
+        issue_g(nxt);
+        g_issued = true;
       }
-      sts16(AB + diag_off, 0);
-      fence_proxy_async_smem();
+      {
+        uint32_t r[2][16];
+        tmem_ld16(acc_t, r[0]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          tmem_wait_ld();
+          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          uint32_t(&c)[16] = r[q & 1];
+          uint32_t p[8];
+          pack16(c, p);
+          if ((((h << 2) + q) >> 1) == wq) set_one(p, dchunk == (h << 2) + q ? dword : 8, dkeep, 0u);
+          tmem_st8(opa_t + 8 * q, p);
+        }
+      }
+      tmem_wait_st();
       tc_fence_before_sync();
-      named_bar_sync(bar_id, kWG);
-      if (t == 0) {
+      named_bar_sync(bar_id, kSlotThreads);
+      if (lead) {
         tc_fence_after_sync();
-        issue_bx(TXd, AB, XB, mma_bar);
+        issue_bx(ACCd, OPAd, XB, mma_bar);
       }
 
       // ---- E3: Xh = (a + B_tt) Xh + offdiag(B) Xh
       mbar_wait(mma_bar, ph_mma);
       ph_mma ^= 1;
       tc_fence_after_sync();
-      if (k + 1 < hp.K) {
+      if (lead && last && step_mode && g_issued) {          // XB is free: fetch the next tile's M
+        issue_m(nxt);
+        m_issued = true;
+      }
+      {
+        const f2 si2 = pk2(si, si);
         f2 Da = pk2(0.f, 0.f), Db = Da;
+        uint32_t r[2][16];
+        tmem_ld16(acc_t, r[0]);
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          uint32_t r[32];
-          tmem_ld32(TX + 32 * g, r);
+        for (int q = 0; q < 4; ++q) {
           tmem_wait_ld();
-          store_group_bf16(xrow, g, r);
+          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          uint32_t(&c)[16] = r[q & 1];
 #pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            const f2 x01 = pk2u(r[4 * j], r[4 * j + 1]), x23 = pk2u(r[4 * j + 2], r[4 * j + 3]);
-            Da = fma2(x01, x01, Da);
-            Db = fma2(x23, x23, Db);
+          for (int j = 0; j < 8; ++j) xs[8 * q + j] = fma2(xs[8 * q + j], si2, pk2u(c[2 * j], c[2 * j + 1]));
+          if (!last) {
+            uint32_t p[8];
+#pragma unroll
+            for (int j = 0; j < 8; j += 2) {
+              Da = fma2(xs[8 * q + j], xs[8 * q + j], Da);
+              Db = fma2(xs[8 * q + j + 1], xs[8 * q + j + 1], Db);
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) p[j] = cvt_bf16x2(xs[8 * q + j]);
+            sts128(chunk_addr(xrow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
+            sts128(chunk_addr(xrow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
+            tmem_st8(opa_t + 8 * q, p);
           }
         }
-        float d0, d1;
-        upk2(add2(Da, Db), d0, d1);
-        di = d0 + d1;
-        sc->dvec[t] = di;
-        fence_proxy_async_smem();
-        tc_fence_before_sync();
-        named_bar_sync(bar_id, kWG);
-        if (t == 0) {
-          tc_fence_after_sync();
-          issue_gram(TAd, XB, 0u, mma_bar);
+        if (!last) {
+          float d0, d1;
+          upk2(add2(Da, Db), d0, d1);
+          sc->dpart[h][t] = d0 + d1;
         }
       }
+      if (!last) {
+        tmem_wait_st();
+        fence_proxy_async_smem();
+        tc_fence_before_sync();
+        named_bar_sync(bar_id, kSlotThreads);
+        if (lead) {
+          tc_fence_after_sync();
+          issue_gram(ACCd, OPAd, XB, 0u, mma_bar);
+        }
+        di = sc->dpart[0][t] + sc->dpart[1][t];
+      }
+    }
+    if (dumped) {   // tests only: return the raw accumulator instead of X_K
+      uint32_t r[16];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        tmem_ld16(acc_t + 16 * q, r);
+        tmem_wait_ld();
+#pragma unroll
+        for (int j = 0; j < 8; ++j) xs[8 * q + j] = pk2u(r[2 * j], r[2 * j + 1]);
+      }
+      tc_fence_before_sync();
     }
 
     // ---------------- F: untile + scaled, weight-decayed write --------------------------------
-    if (mode == MODE_STEP) {
-      if (t == 0) {
-        tma_wait_group_read0();   // M' has left ST
-        mbar_arrive_expect_tx(tma_bar, kTileBytes);
-        tma_load_2d(ST, map_w, x0, y0, tma_bar);
-        tma_load_2d(ST + kHalfBytes, map_w, x0 + 64, y0, tma_bar);
+    if (step_mode) {
+      if (lead && !w_issued) {                               // K = 0 or a debug stage: W was not prefetched
+        tma_wait_group_read0();
+        mbar_arrive_expect_tx(w_bar, kTileBytes);
+        tma_load_2d(ST, map_w, x0, y0, w_bar);
+        tma_load_2d(ST + kHalfBytes, map_w, x0 + 64, y0, w_bar);
       }
-      mbar_wait(tma_bar, ph_tma);
-      ph_tma ^= 1;
-    } else {
-      if (t == 0) tma_wait_group_read0();
-      named_bar_sync(bar_id, kWG);
+      mbar_wait(w_bar, ph_w);
+      ph_w ^= 1;
     }
-    const float keep = 1.f - hp.lr * hp.wd;
-    const float unq = dbg ? 1.f : 1.f / qs;                       // undo the c^(1/4) state scaling
-    const float stepsz = -hp.lr * hp.scale_c * tau_base * unq;
+    {
+      const float keep = 1.f - hp.lr * hp.wd;
+      const float unq = dbg ? 1.f : 1.f / qs;                       // undo the c^(1/4) state scaling
+      const float stepsz = step_mode ? -hp.lr * hp.scale_c * tau_base * unq : unq;
+      const f2 step2 = pk2(stepsz, stepsz), keep2 = pk2(keep, keep);
 #pragma unroll
-    for (int g = 0; g < 4; ++g) {
-      uint32_t r[32];
-      tmem_ld32(out_src + 32 * g, r);
-      tmem_wait_ld();
-      if (mode == MODE_STEP) {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const uint4 wv = lds128(chunk_addr(srow, 4 * g + q));
+      for (int c = 0; c < 8; ++c) {
+        uint32_t p[4];
+        if (step_mode) {
+          const uint4 wv = lds128(chunk_addr(srow, c));
           const uint32_t ww[4] = {wv.x, wv.y, wv.z, wv.w};
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            r[8 * q + 2 * e] = __float_as_uint(fmaf(keep, bf16_lo(ww[e]), stepsz * __uint_as_float(r[8 * q + 2 * e])));
-            r[8 * q + 2 * e + 1] = __float_as_uint(fmaf(keep, bf16_hi(ww[e]), stepsz * __uint_as_float(r[8 * q + 2 * e + 1])));
-          }
-        }
-      } else {
+          for (int e = 0; e < 4; ++e)
+            p[e] = cvt_bf16x2(fma2(keep2, pk2(bf16_lo(ww[e]), bf16_hi(ww[e])), mul2(step2, xs[4 * c + e])));
+        } else {
 #pragma unroll
-        for (int j = 0; j < 32; ++j) r[j] = __float_as_uint(__uint_as_float(r[j]) * unq);
+          for (int e = 0; e < 4; ++e) p[e] = cvt_bf16x2(mul2(step2, xs[4 * c + e]));
+        }
+        sts128(chunk_addr(srow, c), make_uint4(p[0], p[1], p[2], p[3]));
       }
-      store_group_bf16(srow, g, r);
     }
     fence_proxy_async_smem();
-    named_bar_sync(bar_id, kWG);
-    if (t == 0) {
+    named_bar_sync(bar_id, kSlotThreads);
+    if (lead) {
       tma_store_2d(map_w, x0, y0, ST);
       tma_store_2d(map_w, x0 + 64, y0, ST + kHalfBytes);
       tma_commit_group();
+      if (nxt < n_items) {                                   // whatever was not prefetched during the steps
+        if (!g_issued) issue_g(nxt);
+        if (step_mode && !m_issued) issue_m(nxt);
+      }
     }
   }
 
-  if (t == 0) tma_wait_group0();
+  if (lead) tma_wait_group0();
   tc_fence_before_sync();
   __syncthreads();
-  if (tid < 32) tmem_dealloc<512>(tmem_base);
+  if (tid < 32) tmem_dealloc<512>(ctrl->tmem_base);
 }
 
 }  // namespace

@@ -185,6 +185,12 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   const uint32_t bar_id = 1 + slot;
 
   uint32_t ph_mma = 0, ph_ld = 0, ph_w = 0;
+  // One warp of the slot polls the MMA barrier; the others sleep on a hardware barrier, so that waiting
+  // warps do not take issue slots from the other slot's epilogue.
+  auto wait_mma = [&]() {
+    if (w == 0) mbar_wait(mma_bar, ph_mma);
+    named_bar_sync(3 + slot, kSlotThreads);
+  };
   // The state is Xh = c^(1/4) X: then Ah = Xh Xh^T = sqrt(c) A and B = bA + cA^2 = beta Ah + Ah^2 with
   // beta = b / sqrt(c), so the accumulator after MMA2 is B itself (no rescale in E2).
   const float qs = sqrtf(sqrtf(hp.c));
@@ -318,7 +324,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     for (int k = 0; k < hp.K; ++k) {
       const bool last = (k + 1 == hp.K);
       // ---- E1: ACC = Ah = Xh Xh^T just landed
-      mbar_wait(mma_bar, ph_mma);
+      wait_mma();
       ph_mma ^= 1;
       tc_fence_after_sync();
       if (dbg == 1) { dumped = true; break; }
@@ -371,7 +377,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       const float si = hp.a + fmaf(beta_h, di, sc->spart[0][t] + sc->spart[1][t]);
 
       // ---- E2: ACC = B (off-diagonal)
-      mbar_wait(mma_bar, ph_mma);
+      wait_mma();
       ph_mma ^= 1;
       tc_fence_after_sync();
       if (dbg == 2) { dumped = true; break; }
@@ -402,7 +408,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       }
 
       // ---- E3: Xh = (a + B_tt) Xh + offdiag(B) Xh
-      mbar_wait(mma_bar, ph_mma);
+      wait_mma();
       ph_mma ^= 1;
       tc_fence_after_sync();
       if (lead && last && step_mode && g_issued) {          // XB is free: fetch the next tile's M

@@ -18,8 +18,8 @@ CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libhimuon.so")
 STAMP_PATH = os.path.join(PKG_DIR, "libhimuon.stamp")
 
-SOURCES = ["himuon_api.cu", "kernels_simt.cu", "kernels_tc128.cu"]
-HEADERS = ["himuon_internal.h", "sm100_ptx.cuh", os.path.join(ROOT, "include", "himuon.h")]
+SOURCES = ["himuon_api.cu", "kernels_simt.cu", "kernels_tc128.cu", "kernels_tc64.cu"]
+HEADERS = ["himuon_internal.h", "sm100_ptx.cuh", "tc_common.cuh", os.path.join(ROOT, "include", "himuon.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -51,6 +51,8 @@ struct LaunchArgs {
 cudaError_t launch_simt(const LaunchArgs& a, cudaStream_t stream);
 // kernels_tc128.cu -- tcgen05 bf16 path, T = 128, bf16 storage.
 cudaError_t launch_tc128(const LaunchArgs& a, cudaStream_t stream);
+// kernels_tc64.cu -- tcgen05 bf16 path, T = 64 (two tiles stacked per MMA), bf16 storage.
+cudaError_t launch_tc64(const LaunchArgs& a, cudaStream_t stream);
 
 int  device_sm_count();
 void note_launch();

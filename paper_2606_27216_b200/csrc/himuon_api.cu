@@ -35,6 +35,7 @@ int select_kpath(int dtype, int path, int T, int W = 0) {
   if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : -1;
   // bf16 storage, AUTO: tensor-core path where it exists, else the fp32 kernel.
   if ((T == 128 || T == 64) && (W % 8) == 0) return KPATH_TC;
+  if (T == 16 || T == 32) return KPATH_WARP;
   return simt_ok ? KPATH_FP32_SIMT : -1;
 }
 
@@ -113,6 +114,7 @@ himuon_status chunk_rule(long long n_items, long long bytes_per_item, long long 
 cudaError_t launch_chunk(const LaunchArgs& a, int kpath, cudaStream_t s) {
   g_launches.fetch_add(1);
   if (kpath == KPATH_TC) return a.T == 64 ? launch_tc64(a, s) : launch_tc128(a, s);
+  if (kpath == KPATH_WARP) return launch_warp(a, s);
   return launch_simt(a, s);
 }
 

@@ -34,7 +34,7 @@ struct WorkItem {
 static_assert(sizeof(WorkItem) == 16, "WorkItem must be 16 bytes");
 
 enum Mode : int { MODE_STEP = 0, MODE_PHI = 1 };
-enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1 };
+enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1, KPATH_WARP = 2 };
 
 struct LaunchArgs {
   const LayerDev*    layers;     // device
@@ -53,6 +53,8 @@ cudaError_t launch_simt(const LaunchArgs& a, cudaStream_t stream);
 cudaError_t launch_tc128(const LaunchArgs& a, cudaStream_t stream);
 // kernels_tc64.cu -- tcgen05 bf16 path, T = 64 (two tiles stacked per MMA), bf16 storage.
 cudaError_t launch_tc64(const LaunchArgs& a, cudaStream_t stream);
+// kernels_warp.cu -- mma.sync bf16 path, one warp per tile, T in {16, 32}, bf16 storage.
+cudaError_t launch_warp(const LaunchArgs& a, cudaStream_t stream);
 
 int  device_sm_count();
 void note_launch();

@@ -91,6 +91,15 @@ struct TileIO {
       if (col + 1 < W) hi = __bfloat162float(q[1]);
     }
   }
+  // the same pair as stored bits (lo in the low half), zero outside the matrix
+  __device__ __forceinline__ uint32_t load2_raw(int row, int col) const {
+    if (row >= H || col >= W) return 0u;
+    const __nv_bfloat16* q = p + (long long)row * ld + col;
+    if (fast && col + 1 < W) return __ldg(reinterpret_cast<const uint32_t*>(q));
+    uint32_t u = *reinterpret_cast<const unsigned short*>(q);
+    if (col + 1 < W) u |= (uint32_t)(*reinterpret_cast<const unsigned short*>(q + 1)) << 16;
+    return u;
+  }
   __device__ __forceinline__ void store2(int row, int col, float lo, float hi) const {
     if (row >= H || col >= W) return;
     __nv_bfloat16* q = p + (long long)row * ld + col;
@@ -257,44 +266,67 @@ himuon_warp_kernel(const LayerDev* __restrict__ layers, const WorkItem* __restri
   const float beta_h = hp.b / sqrtf(hp.c);
   const long long stride = (long long)gridDim.x * kWarpsPerBlock;
 
-  for (long long it = (long long)blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5); it < n_items; it += stride) {
+  // Software pipeline over the warp's tiles: the work item, the layer descriptor and the raw G / M bits of
+  // the NEXT tile are requested before the Newton-Schulz steps of the current one, and W of the current
+  // tile before its steps, so that the dependent chain item -> layer -> data never stalls the warp.
+  auto fetch = [&](long long i, LayerDev& L, int& row0, int& col0, uint32_t (&gq)[NB * NB * 4], uint32_t (&mq)[NB * NB * 4]) {
     WorkItem wi;
-    if (items) wi = items[it];
-    else { wi.layer = 0; wi.r = (int)it; wi.c = 0; wi.pad = 0; }
-    const LayerDev L = layers[wi.layer];
-    const int row0 = wi.r * T, col0 = wi.c * T;
+    if (items) wi = items[i];
+    else { wi.layer = 0; wi.r = (int)i; wi.c = 0; wi.pad = 0; }
+    L = layers[wi.layer];
+    row0 = wi.r * T;
+    col0 = wi.c * T;
     const TileIO ioG = make_io(L.g, L.ld_g, L.H, L.W);
+    const TileIO ioM = make_io(L.m, L.ld_m, L.H, L.W);
+#pragma unroll
+    for (int q = 0; q < NB * NB * 4; ++q) {
+      const int i2 = q / (NB * 4), j2 = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
+      const int row = row0 + 16 * i2 + g + 8 * rr, col = col0 + 16 * j2 + 8 * nh + 2 * c;
+      gq[q] = ioG.load2_raw(row, col);
+      mq[q] = step_mode ? ioM.load2_raw(row, col) : 0u;
+    }
+  };
+
+  long long it = (long long)blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  LayerDev Ln;
+  int rown = 0, coln = 0;
+  uint32_t gq[NB * NB * 4], mq[NB * NB * 4];
+  if (it < n_items) fetch(it, Ln, rown, coln, gq, mq);
+
+  while (it < n_items) {
+    const LayerDev L = Ln;
+    const int row0 = rown, col0 = coln;
     const TileIO ioM = make_io(L.m, L.ld_m, L.H, L.W);
     const TileIO ioW = make_io(L.w, L.ld_w, L.H, L.W);
 
-    // ---------------- P: load, momentum, Frobenius normalisation ----
+    // ---------------- P: momentum, Frobenius normalisation ----------
     Blk x[NB][NB];
     float ss = 0.f;
 #pragma unroll
-    for (int i = 0; i < NB; ++i)
+    for (int q = 0; q < NB * NB * 4; ++q) {
+      const int i = q / (NB * 4), j = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
+      const int row = row0 + 16 * i + g + 8 * rr, col = col0 + 16 * j + 8 * nh + 2 * c;
+      const float g0 = __uint_as_float(gq[q] << 16), g1 = __uint_as_float(gq[q] & 0xffff0000u);
+      float h0 = g0, h1 = g1;
+      if (step_mode) {
+        const float m0 = fmaf(hp.beta, __uint_as_float(mq[q] << 16), g0);
+        const float m1 = fmaf(hp.beta, __uint_as_float(mq[q] & 0xffff0000u), g1);
+        ioM.store2(row, col, m0, m1);
+        h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;
+        h1 = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
+      }
+      x[i][j].v[nh][2 * rr] = h0;
+      x[i][j].v[nh][2 * rr + 1] = h1;
+      ss = fmaf(h0, h0, fmaf(h1, h1, ss));
+    }
+    const long long nx = it + stride;
+    if (nx < n_items) fetch(nx, Ln, rown, coln, gq, mq);      // consumed in the next iteration
+    uint32_t wq[NB * NB * 4];                                  // W of this tile, consumed after the steps
 #pragma unroll
-      for (int j = 0; j < NB; ++j)
-#pragma unroll
-        for (int nh = 0; nh < 2; ++nh)
-#pragma unroll
-          for (int rr = 0; rr < 2; ++rr) {
-            const int row = row0 + 16 * i + g + 8 * rr, col = col0 + 16 * j + 8 * nh + 2 * c;
-            float g0, g1;
-            ioG.load2(row, col, g0, g1);
-            float h0 = g0, h1 = g1;
-            if (step_mode) {
-              float m0, m1;
-              ioM.load2(row, col, m0, m1);
-              m0 = fmaf(hp.beta, m0, g0);
-              m1 = fmaf(hp.beta, m1, g1);
-              ioM.store2(row, col, m0, m1);
-              h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;
-              h1 = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
-            }
-            x[i][j].v[nh][2 * rr] = h0;
-            x[i][j].v[nh][2 * rr + 1] = h1;
-            ss = fmaf(h0, h0, fmaf(h1, h1, ss));
-          }
+    for (int q = 0; q < NB * NB * 4; ++q) {
+      const int i = q / (NB * 4), j = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
+      wq[q] = step_mode ? ioW.load2_raw(row0 + 16 * i + g + 8 * rr, col0 + 16 * j + 8 * nh + 2 * c) : 0u;
+    }
     float tot = ss;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
@@ -330,23 +362,17 @@ himuon_warp_kernel(const LayerDev* __restrict__ layers, const WorkItem* __restri
     const float unq = 1.f / qs;
     const float stepsz = step_mode ? -hp.lr * hp.scale_c * L.tau_base * unq : unq;
 #pragma unroll
-    for (int i = 0; i < NB; ++i)
-#pragma unroll
-      for (int j = 0; j < NB; ++j)
-#pragma unroll
-        for (int nh = 0; nh < 2; ++nh)
-#pragma unroll
-          for (int rr = 0; rr < 2; ++rr) {
-            const int row = row0 + 16 * i + g + 8 * rr, col = col0 + 16 * j + 8 * nh + 2 * c;
-            float o0 = stepsz * x[i][j].v[nh][2 * rr], o1 = stepsz * x[i][j].v[nh][2 * rr + 1];
-            if (step_mode) {
-              float w0, w1;
-              ioW.load2(row, col, w0, w1);
-              o0 = fmaf(keep, w0, o0);
-              o1 = fmaf(keep, w1, o1);
-            }
-            ioW.store2(row, col, o0, o1);
-          }
+    for (int q = 0; q < NB * NB * 4; ++q) {
+      const int i = q / (NB * 4), j = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
+      const int row = row0 + 16 * i + g + 8 * rr, col = col0 + 16 * j + 8 * nh + 2 * c;
+      float o0 = stepsz * x[i][j].v[nh][2 * rr], o1 = stepsz * x[i][j].v[nh][2 * rr + 1];
+      if (step_mode) {
+        o0 = fmaf(keep, __uint_as_float(wq[q] << 16), o0);
+        o1 = fmaf(keep, __uint_as_float(wq[q] & 0xffff0000u), o1);
+      }
+      ioW.store2(row, col, o0, o1);
+    }
+    it = nx;
   }
 }
 

@@ -34,7 +34,7 @@ int select_kpath(int dtype, int path, int T, int W = 0) {
   const bool simt_ok = (T == 16 || T == 32 || T == 64 || T == 128);
   if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : -1;
   // bf16 storage, AUTO: tensor-core path where it exists, else the fp32 kernel.
-  if ((T == 128 || T == 64) && (W % 8) == 0) return KPATH_TC;
+  if ((T == 256 || T == 128 || T == 64) && (W % 8) == 0) return KPATH_TC;
   if (T == 16 || T == 32) return KPATH_WARP;
   return simt_ok ? KPATH_FP32_SIMT : -1;
 }
@@ -113,7 +113,7 @@ himuon_status chunk_rule(long long n_items, long long bytes_per_item, long long 
 
 cudaError_t launch_chunk(const LaunchArgs& a, int kpath, cudaStream_t s) {
   g_launches.fetch_add(1);
-  if (kpath == KPATH_TC) return a.T == 64 ? launch_tc64(a, s) : launch_tc128(a, s);
+  if (kpath == KPATH_TC) return a.T == 64 ? launch_tc64(a, s) : a.T == 256 ? launch_tc256(a, s) : launch_tc128(a, s);
   if (kpath == KPATH_WARP) return launch_warp(a, s);
   return launch_simt(a, s);
 }
@@ -213,6 +213,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       Te = T;
     }
     const int kp = select_kpath(dt, path, Te, W);
+    if (kp < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }   // e.g. T = 256 on a bf16 width that is not a multiple of 8
     p->T_eff[l] = Te;
     p->kpath[l] = kp;
     if (!L.g.ptr || !L.w.ptr) p->bindable = false;
@@ -340,7 +341,7 @@ himuon_status himuon_plan_bind(himuon_plan* plan, void* workspace, size_t worksp
       const himuon_mat*   ms[3] = {&L.w, &L.g, &L.m};
       for (int i = 0; i < 3; ++i) {
         if (!ms[i]->ptr) continue;
-        if (!encode_bf16_map(&maps[(size_t)l * 3 + i], ms[i]->ptr, ms[i]->H, ms[i]->W, ms[i]->ld, plan->T_eff[l])) {
+        if (!encode_bf16_map(&maps[(size_t)l * 3 + i], ms[i]->ptr, ms[i]->H, ms[i]->W, ms[i]->ld, plan->T_eff[l] > 128 ? 128 : plan->T_eff[l])) {
           g_last_cuda_error = "bind: cuTensorMapEncodeTiled failed or unavailable";
           return HIMUON_ERR_CUDA;
         }
@@ -444,7 +445,7 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
   if (kp == KPATH_TC) {
     CUtensorMap maps[3];
     std::memset(maps, 0, sizeof(maps));
-    if (!encode_bf16_map(&maps[0], D.w, D.H, D.W, T, T) || !encode_bf16_map(&maps[1], D.g, D.H, D.W, T, T)) {
+    if (!encode_bf16_map(&maps[0], D.w, D.H, D.W, T, T > 128 ? 128 : T) || !encode_bf16_map(&maps[1], D.g, D.H, D.W, T, T > 128 ? 128 : T)) {
       g_last_cuda_error = "ns_tiles: cuTensorMapEncodeTiled failed or unavailable";
       return HIMUON_ERR_CUDA;
     }

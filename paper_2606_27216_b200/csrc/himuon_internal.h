@@ -53,6 +53,8 @@ cudaError_t launch_simt(const LaunchArgs& a, cudaStream_t stream);
 cudaError_t launch_tc128(const LaunchArgs& a, cudaStream_t stream);
 // kernels_tc64.cu -- tcgen05 bf16 path, T = 64 (two tiles stacked per MMA), bf16 storage.
 cudaError_t launch_tc64(const LaunchArgs& a, cudaStream_t stream);
+// kernels_tc256.cu -- tcgen05 cta_group::2 bf16 path, T = 256 (one tile per CTA pair), bf16 storage.
+cudaError_t launch_tc256(const LaunchArgs& a, cudaStream_t stream);
 // kernels_warp.cu -- mma.sync bf16 path, one warp per tile, T in {16, 32}, bf16 storage.
 cudaError_t launch_warp(const LaunchArgs& a, cudaStream_t stream);
 

@@ -226,24 +226,38 @@ def run_gpu(args):
     if rank != 0:
         return
     pk = peaks()
-    kern_ms = statistics.mean(per_step) / max(1, plan.n_chunks)     # dominant kernel = the fused step kernel
-    ach = flops / plan.n_chunks / (kern_ms * 1e-3) / 1e12
+    # dominant kernel = the fused step kernel of the plan-wide tile size (one launch per chunk)
+    kname = {16: "himuon_warp_kernel", 32: "himuon_warp_kernel", 64: "himuon_tc64_kernel", 128: "himuon_tc128_kernel",
+             256: "himuon_tc256_kernel"}.get(args.T, "himuon_simt_kernel")
+    kern_ms = statistics.mean(per_step) / max(1, plan.n_chunks)
     bytes_step = 10.0 * n_elem
+    t_tensor = flops / (pk["bf16_sustained"] * 1e12)
+    t_hbm = bytes_step / (pk["hbm_gbs"] * 1e9)
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(f"{args.workload}:T{args.T}")
-    roof = {"bound": "tensor", "achieved": round(ach, 2), "peak": pk["bf16_sustained"], "unit": "TFLOP/s",
-            "frac": round(ach / pk["bf16_sustained"], 4), "traffic": traffic,
-            "peak_kind": "sustained bf16, " + pk["source"], "frac_of_burst": round(ach / pk["bf16_burst"], 4),
-            "kernel": "himuon_tc128_kernel", "launch_ms": round(kern_ms, 4),
-            "hbm_gbs_achieved": round(bytes_step / (ms_per_step * 1e-3) / 1e9, 1), "hbm_frac": round(bytes_step / (ms_per_step * 1e-3) / 1e9 / pk["hbm_gbs"], 4),
-            "roofline_ms": round(max(flops / (pk["bf16_sustained"] * 1e12), bytes_step / (pk["hbm_gbs"] * 1e9)) * 1e3, 3)}
+    tp = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    if os.path.exists(tp):                                    # measured DRAM bytes per element (ncu) x elements per launch
+        for ln in open(tp).read().splitlines()[1:]:
+            f = ln.split(",")
+            if f[0] == kname and int(f[1]) == args.T and not any(l.T for l in spec.layers):
+                traffic = float(f[5]) * n_elem / plan.n_chunks
+    if t_tensor >= t_hbm:
+        ach = flops / plan.n_chunks / (kern_ms * 1e-3) / 1e12
+        roof = {"bound": "tensor", "achieved": round(ach, 2), "peak": pk["bf16_sustained"], "unit": "TFLOP/s",
+                "frac": round(ach / pk["bf16_sustained"], 4), "traffic": traffic,
+                "peak_kind": "sustained bf16, " + pk["source"], "frac_of_burst": round(ach / pk["bf16_burst"], 4)}
+    else:
+        ach = bytes_step / plan.n_chunks / (kern_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": round(ach, 1), "peak": pk["hbm_gbs"], "unit": "GB/s",
+                "frac": round(ach / pk["hbm_gbs"], 4), "traffic": traffic, "peak_kind": "copy bandwidth, " + pk["source"]}
+    roof.update({"kernel": kname, "launch_ms": round(kern_ms, 4),
+                 "tflops_achieved": round(flops / (ms_per_step * 1e-3) / 1e12, 2),
+                 "hbm_gbs_achieved": round(bytes_step / (ms_per_step * 1e-3) / 1e9, 1),
+                 "roofline_ms": round(max(t_tensor, t_hbm) * 1e3, 3)})
     cpu = run_cpu_baseline(args, spec, hp)
     line = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": {"workload": f"{spec.name}-shaped HiMuon step (BASELINE configs[4])" if spec.name == "llama3-8b" else f"{spec.name}-shaped HiMuon step",
+            "config": {"workload": f"{spec.name}-shaped HiMuon step (BASELINE configs[4])" if spec.name.startswith("llama3-8b") else f"{spec.name}-shaped HiMuon step",
                        "layers": len(spec.layers), "elements": n_elem, "tiles": plan.n_tiles, "T": args.T, "K": args.K,
                        "chunks": plan.n_chunks, "workspace_bytes": plan.workspace_bytes, "cap_mb": args.cap_mb,
                        "l2": "inputs (%.1f GB) larger than L2" % (bytes_step / 1e9), "parallelism": f"replicas x{world}, no collective",

@@ -175,7 +175,12 @@ def run_gpu(args):
         spec.layers = spec.layers[: per_block * args.blocks]
         spec.name += f"[first {args.blocks} blocks]"
     hp = hm.HParams(K=args.K, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
-    Ws, Gs, Ms = make_inputs(spec, dev)                       # weak scaling: every rank owns a full parameter set
+    flops_job = algorithmic_flops(spec, args.T, args.K) * (1 if args.shard else world)
+    if args.shard and world > 1:                              # strong scaling: whole matrices per rank, no collective
+        from paper_2606_27216_b200.shard import shard_layers
+        mine = shard_layers([l.H * l.W for l in spec.layers], world)[rank]
+        spec.layers = [spec.layers[i] for i in mine]
+    Ws, Gs, Ms = make_inputs(spec, dev)                       # default (weak scaling): every rank owns a full parameter set
     Tl = [l.T for l in spec.layers]
     plan = hm.Plan.from_tensors(Ws, Gs, Ms, args.T, T_per_layer=Tl if any(Tl) else None,
                                 workspace_cap_bytes=args.cap_mb << 20).bind()
@@ -218,7 +223,7 @@ def run_gpu(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
     ms_per_step = total_ms / args.steps
-    value = world * flops / (ms_per_step * 1e-3) / 1e12
+    value = flops_job / (ms_per_step * 1e-3) / 1e12
 
     # ---- e2e: same metric through the public API with HOST buffers (gradients in, weights out)
     e2e = run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier)
@@ -256,11 +261,11 @@ def run_gpu(args):
     cpu = run_cpu_baseline(args, spec, hp)
     line = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "scaling": "strong" if args.shard else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": f"{spec.name}-shaped HiMuon step (BASELINE configs[4])" if spec.name.startswith("llama3-8b") else f"{spec.name}-shaped HiMuon step",
                        "layers": len(spec.layers), "elements": n_elem, "tiles": plan.n_tiles, "T": args.T, "K": args.K,
                        "chunks": plan.n_chunks, "workspace_bytes": plan.workspace_bytes, "cap_mb": args.cap_mb,
-                       "l2": "inputs (%.1f GB) larger than L2" % (bytes_step / 1e9), "parallelism": f"replicas x{world}, no collective",
+                       "l2": "inputs (%.1f GB) larger than L2" % (bytes_step / 1e9), "parallelism": (f"whole matrices sharded over {world} ranks" if args.shard else f"replicas x{world}") + ", no collective",
                        "gflop_per_step": round(flops / 1e9, 1)},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
             "step_ms_median": round(statistics.median(per_step), 4), "step_ms_min": round(min(per_step), 4)}
@@ -370,6 +375,7 @@ def main():
     ap.add_argument("--cpu-tiles", type=int, default=4096)
     ap.add_argument("--e2e-host-gb", type=float, default=8.0)
     ap.add_argument("--blocks", type=int, default=0, help="truncate the parameter set to its first N transformer blocks (profiling only)")
+    ap.add_argument("--shard", action="store_true", help="N > 1: split the parameter set over the ranks by whole matrices (strong scaling)")
     ap.add_argument("--suite", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -10,8 +10,8 @@
 //                                  B operand is the stacked X' read MN-major, N = 2 x 64)
 // Half of each MMA is wasted; the epilogues touch only the useful 64 accumulator columns of a row, so
 // CUDA-core work per matrix element equals that of the T = 128 kernel.  Everything else (operands in
-// TMEM, fp32 iterate in registers, fp32 diagonal of B as a row scaling, TMA prefetch, two independent
-// slots per CTA) follows kernels_tc128.cu, whose header states the per-tile algorithm and its citations.
+// TMEM, fp32 iterate in registers, fp32 diagonal of B as a row scaling, TMA prefetch, independent slots per
+// CTA - three here, since a slot needs only 48 KB of shared memory, 160 TMEM columns and 32 state registers) follows kernels_tc128.cu, whose header states the per-tile algorithm and its citations.
 //
 // Thread (t, h) of a slot: row t of the super-tile (tile b = t >> 6, TMEM lane t), column half h of that
 // tile (columns 32h..32h+31, i.e. accumulator columns 64b + 32h ..).
@@ -30,7 +30,7 @@ using namespace tc;
 
 constexpr int T = 64;
 constexpr int kPack = 2;                         // tiles per super-tile
-constexpr int kSlots = 2;
+constexpr int kSlots = 3;                        // independent super-tiles in flight per CTA (TMEM: 3 x 160 columns)
 constexpr int kSlotThreads = 256;                // 8 warps: 4 lane quadrants x 2 column halves
 constexpr int kThreads = kSlots * kSlotThreads;
 constexpr uint32_t kTileBytes = T * T * 2;       // 8 KB: one bf16 tile = 64 rows x 128 B (one swizzle span wide)
@@ -38,7 +38,7 @@ constexpr uint32_t kBufBytes = kPack * kTileBytes;   // 16 KB: a stacked 128 x 6
 constexpr uint32_t kSlotBytes = 3 * kBufBytes;   // XB, OB, ST
 constexpr uint32_t kCtrlBytes = 8192;
 constexpr uint32_t kSmemBytes = kSlots * kSlotBytes + kCtrlBytes + 1024;  // + alignment slack
-constexpr uint32_t kSlotCols = 256;              // TMEM columns per slot: ACC 128 (fp32) + OPA 32 (bf16 pairs)
+constexpr uint32_t kSlotCols = 160;              // TMEM columns per slot: ACC 128 (fp32) + OPA 32 (bf16 pairs)
 constexpr uint32_t kOpaCol = 128;
 
 struct SlotCtrl {
@@ -135,7 +135,7 @@ himuon_tc64_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __res
   uint32_t ph_mma = 0, ph_ld = 0, ph_w = 0;
   auto wait_mma = [&]() {   // one warp polls, the others sleep on a hardware barrier
     if (w == 0) mbar_wait(mma_bar, ph_mma);
-    named_bar_sync(3 + slot, kSlotThreads);
+    named_bar_sync(8 + slot, kSlotThreads);
     ph_mma ^= 1;
     tc_fence_after_sync();
   };

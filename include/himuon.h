@@ -49,9 +49,15 @@ typedef enum {
 typedef enum { HIMUON_F32 = 0, HIMUON_BF16 = 1 } himuon_dtype;
 
 /* Kernel path (PAPER.md:233 buckets tiles by "tile shape, dtype and kernel path").
- *   AUTO : bf16 storage -> tensor-core path (bf16 MMA operands, fp32 accumulation, fp32 X state);
+ *   AUTO : bf16 storage -> tensor-core path (bf16 MMA operands, fp32 accumulation, fp32 X state):
+ *            T = 16, 32   one warp per tile, mma.sync, registers only      (any width / ld)
+ *            T = 64       tcgen05, two tiles stacked per 128-lane MMA      (W % 8 == 0, ptr and ld*2 16-byte aligned)
+ *            T = 128      tcgen05, operands and accumulator in TMEM        (same)
+ *            T = 256      tcgen05 cta_group::2, one tile per CTA pair      (same)
+ *          a bf16 matrix whose width is not a multiple of 8 is served by the fp32 kernel at T = 64, 128 and is
+ *          HIMUON_ERR_UNSUPPORTED at T = 256;
  *          fp32 storage -> fp32 path.
- *   FP32 : true fp32 FMA arithmetic for any storage dtype (the <= 1e-4 path). */
+ *   FP32 : true fp32 FMA arithmetic for any storage dtype, T in {16, 32, 64, 128} (the <= 1e-4 path). */
 typedef enum { HIMUON_PATH_AUTO = 0, HIMUON_PATH_FP32 = 1 } himuon_path;
 
 /* {ptr, H, W, ld, dtype}: one row-major device matrix. */

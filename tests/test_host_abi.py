@@ -168,3 +168,28 @@ def test_tma_alignment_is_checked():
         hm.Plan([hm.himuon_layer(hm.himuon_mat(256, 256, 256, 257, 1), hm.himuon_mat(256, 256, 256, 257, 1),
                                  hm.himuon_mat(256, 256, 256, 257, 1), 0)], 128)
     assert e.value.status == B.HIMUON_ERR_UNSUPPORTED
+
+
+def test_supported_tile_sizes_per_dtype_and_path():
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_F32) == [16, 32, 64, 128]
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16) == [16, 32, 64, 128, 256]
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16, hm.HIMUON_PATH_FP32) == [16, 32, 64, 128]
+    with pytest.raises(hm.HimuonError) as e:
+        hm.Plan(_layers([(512, 512)], hm.HIMUON_F32), 256)      # no fp32 kernel for T = 256
+    assert e.value.status == B.HIMUON_ERR_UNSUPPORTED
+    with pytest.raises(hm.HimuonError) as e:
+        hm.Plan(_layers([(512, 300)]), 256)                     # bf16 T = 256 needs a width that is a multiple of 8
+    assert e.value.status == B.HIMUON_ERR_UNSUPPORTED
+    assert hm.Plan(_layers([(512, 512)]), 256).n_tiles == 4
+    assert hm.Plan(_layers([(200, 256)]), 256).n_tiles == 1     # full-matrix branch served by the T = 256 kernel
+
+
+def test_kernel_paths_bucket_the_work_list():
+    """Buckets by (T, dtype, kernel path): bf16 T = 16/32 -> warp kernel, 64/128/256 -> tcgen05
+    kernels, a bf16 width that is not a multiple of 8 -> fp32 kernel; one bucket per distinct key."""
+    shapes = [(256, 256), (256, 256), (256, 256), (256, 256), (256, 256), (256, 250)]
+    p = hm.Plan(_layers(shapes, Ts=[16, 32, 64, 128, 256, 128]), 128)
+    assert p.n_buckets == 6
+    assert p.n_tiles == 256 + 64 + 16 + 4 + 1 + 4
+    _, offs, cT = p.worklist()
+    assert cT.tolist() == [16, 32, 64, 128, 256, 128] and p.n_chunks == 6

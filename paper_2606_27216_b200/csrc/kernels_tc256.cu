@@ -27,6 +27,15 @@
 #include "tc_common.cuh"
 
 namespace himuon {
+
+#ifdef HIMUON_TRACE   // development aid (not built into libhimuon.so): clock stamps of thread 0 of CTA 0
+__device__ long long g_trace[2][8192];
+__device__ int g_tn;
+#define TR() do { if (threadIdx.x == 0 && blockIdx.x == 0 && g_tn < 8192) g_trace[0][g_tn++] = clock64(); } while (0)
+#else
+#define TR() do { } while (0)
+#endif
+
 namespace {
 
 using namespace ptx;
@@ -98,9 +107,11 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   const uint32_t XB = smem0, OB = XB + kBufBytes, ST = OB + kBufBytes;
   const uint32_t rowoff = (uint32_t)q4 * kBlkBytes + (uint32_t)t * 128u + ((uint32_t)(t & 7) << 4);
   const uint32_t xrow = XB + rowoff, orow = OB + rowoff, srow = ST + rowoff;
-  // this thread's 64 columns of row R in the MN-major copy of Xb: CTA q4 >> 1, atom q4 & 1, K-row R
-  const uint32_t xt_local = OB + (uint32_t)(q4 & 1) * kAtomBytes + (uint32_t)R * 128u + ((uint32_t)(R & 7) << 4);
-  const uint32_t xt_row = mapa_shared(xt_local, (uint32_t)(q4 >> 1));
+  // this thread's 64 columns of row R in the MN-major (column-split) copy of Xb, which lives in the staging
+  // buffer ST during the steps: CTA q4 >> 1, atom q4 & 1, K-row R
+  const uint32_t xt_local = ST + (uint32_t)(q4 & 1) * kAtomBytes + (uint32_t)R * 128u + ((uint32_t)(R & 7) << 4);
+  const bool xt_is_local = ((uint32_t)(q4 >> 1) == rank);              // warp-uniform
+  const uint32_t xt_row = xt_is_local ? xt_local : mapa_shared(xt_local, (uint32_t)(q4 >> 1));
   const uint32_t mma_bar = smem_u32(&ctrl->mma_bar);
   const uint32_t ready_bar = smem_u32(&ctrl->ready_bar);
   const uint32_t ready_bar_leader = mapa_shared(ready_bar, 0);
@@ -110,7 +121,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   if (tid == 0) {
     mbar_init(mma_bar, 1);
     mbar_init(ready_bar, 2);
-    mbar_init(ld_bar, 1);
+    mbar_init(ld_bar, 2);   // arrive.expect_tx at issue + "staging buffer is free" arrive of the lead thread
     mbar_init(w_bar, 1);
     fence_mbar_init();
   }
@@ -130,7 +141,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   const float beta_h = hp.b / sqrtf(hp.c);
 
   // Operands of the next pair MMA are written: tell the leader; the leader issues once both CTAs have.
-  // which: 1 = MMA1 (B = XB, K-major), 2 = MMA2 (B = OB, K-major), 3 = MMA3 (B = Xb copy in OB, MN-major).
+  // which: 1 = MMA1 (B = XB, K-major), 2 = MMA2 (B = OB, K-major), 3 = MMA3 (B = Xb copy in ST, MN-major).
   auto ready_and_issue = [&](int which) {
     tmem_wait_st();
     fence_proxy_async_all();          // generic-proxy writes (local and remote smem) -> visible to the MMA
@@ -141,7 +152,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       if (rank == 0) {
         mbar_wait_cluster(ready_bar, ph_ready);
         tc_fence_after_sync();
-        issue_pair(ACCd, OPAd, which == 1 ? XB : OB, which == 3, mma_bar);
+        issue_pair(ACCd, OPAd, which == 1 ? XB : which == 2 ? OB : ST, which == 3, mma_bar);
       }
     }
     ph_ready ^= 1;
@@ -153,29 +164,63 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     tc_fence_after_sync();
   };
 
+#ifdef HIMUON_TRACE
+  if (threadIdx.x == 0 && blockIdx.x == 0) g_tn = 0;
+#endif
+  // The column-split bf16 copy of the iterate that MMA3 reads (into ST of the owning CTA).  Called right after
+  // MMA1 has been issued, i.e. off the critical path: the stores (half of them remote) overlap the MMA.
+  auto write_xb_copy = [&](const f2 (&xs)[32]) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      uint32_t x8[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) x8[j] = cvt_bf16x2(xs[8 * q + j]);
+      if (xt_is_local) {
+        sts128(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
+        sts128(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
+      } else {
+        st_cluster_v4(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
+        st_cluster_v4(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
+      }
+    }
+  };
+
+  // G -> OB and (step mode) M -> XB of tile i: this CTA's 128 rows, four 64-column boxes each
+  auto issue_gm = [&](long long i) {
+    WorkItem wn;
+    if (items) wn = items[i];
+    else { wn.layer = 0; wn.r = (int)i; wn.c = 0; wn.pad = 0; }
+    const int xn = wn.c * T, yn = wn.r * T + (int)rank * kRows;
+    mbar_arrive_expect_tx(ld_bar, step_mode ? 2 * kBufBytes : kBufBytes);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      tma_load_2d(OB + j * kBlkBytes, tmaps + 3 * wn.layer + 1, xn + 64 * j, yn, ld_bar);
+      if (step_mode) tma_load_2d(XB + j * kBlkBytes, tmaps + 3 * wn.layer + 2, xn + 64 * j, yn, ld_bar);
+    }
+  };
+  bool prefetched = false;   // every thread tracks it (uniform); only the lead thread issues
+
   for (long long it = cluster_id_x(); it < n_items; it += cluster_count_x()) {
+    TR();   // tile start
     WorkItem wi;
     if (items) wi = items[it];
     else { wi.layer = 0; wi.r = (int)it; wi.c = 0; wi.pad = 0; }
     const float tau_base = layers[wi.layer].tau_base;
     const CUtensorMap* map_w = tmaps + 3 * wi.layer + 0;
-    const CUtensorMap* map_g = tmaps + 3 * wi.layer + 1;
     const CUtensorMap* map_m = tmaps + 3 * wi.layer + 2;
     const int x0 = wi.c * T, y0 = wi.r * T + (int)rank * kRows;
     bool w_issued = false;
+    const long long nxt = it + cluster_count_x();
 
     // ---------------- P: load, momentum, normalise ---------------------------------------------------
     if (lead) {
-      tma_wait_group_read0();   // the previous tile's stores out of ST have been read
-      mbar_arrive_expect_tx(ld_bar, step_mode ? 2 * kBufBytes : kBufBytes);
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        tma_load_2d(OB + j * kBlkBytes, map_g, x0 + 64 * j, y0, ld_bar);
-        if (step_mode) tma_load_2d(XB + j * kBlkBytes, map_m, x0 + 64 * j, y0, ld_bar);
-      }
+      if (!prefetched) issue_gm(it);
+      tma_wait_group_read0();   // the previous tile's stores out of ST have been read: M' may be written into it
+      mbar_arrive(ld_bar);
     }
     mbar_wait(ld_bar, ph_ld);
     ph_ld ^= 1;
+    prefetched = false;
 
     f2 xs[32];                  // fp32 state: this thread's 64 columns of row R, as packed pairs
     f2 ss2 = pk2(0.f, 0.f);
@@ -224,6 +269,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
 #pragma unroll
         for (int j = 0; j < 4; ++j) tma_store_2d(map_m, x0 + 64 * j, y0, ST + j * kBlkBytes);
         tma_commit_group();
+        tma_wait_group_read0();   // after the cluster barrier below, ST of BOTH CTAs may receive the Xb copy
       }
       st_cluster_f32(mapa_shared(smem_u32(&ctrl->peer_ss), rank ^ 1u), mine);   // Frobenius norm spans both CTAs
     }
@@ -247,8 +293,11 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         tmem_st8(opa_t + 8 * q, p);
       }
     }
+    TR();   // prologue compute done
     if (hp.K > 0) ready_and_issue(1);
     else __syncthreads();
+    TR();   // MMA1 issued
+    if (hp.K > 0) write_xb_copy(xs);
     float di = (ctrl->dpart[0][t] + ctrl->dpart[1][t]) + (ctrl->dpart[2][t] + ctrl->dpart[3][t]);
 
     // ---------------- K Newton-Schulz steps ---------------------------------------------------
@@ -257,6 +306,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       const bool last = (k + 1 == hp.K);
       // ---- E1: ACC = rows of Ah
       wait_mma();
+      TR();   // MMA1 done
       {
         // Ot = offdiag(Ah) + diag(d + beta/2), rounded to bf16: offdiag(Ot Ot^T) = offdiag(beta Ah + Ah^2)
         const uint32_t dval = (pack_bf16(fmaf(0.5f, beta_h, di), 0.f) & 0xffffu) << ((t & 1) * 16);
@@ -285,19 +335,15 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         upk2(add2(Sa, Sb), s0, s1);
         ctrl->spart[q4][t] = s0 + s1;
       }
-      if (lead && step_mode && !w_issued) {                 // M' has left ST by now: fetch W into it
-        tma_wait_group_read0();
-        mbar_arrive_expect_tx(w_bar, kBufBytes);
-#pragma unroll
-        for (int j = 0; j < 4; ++j) tma_load_2d(ST + j * kBlkBytes, map_w, x0 + 64 * j, y0, w_bar);
-        w_issued = true;
-      }
+      TR();   // E1 loop done
       ready_and_issue(2);
+      TR();   // MMA2 issued
       // a + B_RR, B_RR = beta d_R + (Ah^2)_RR
       const float si = hp.a + fmaf(beta_h, di, (ctrl->spart[0][t] + ctrl->spart[1][t]) + (ctrl->spart[2][t] + ctrl->spart[3][t]));
 
-      // ---- E2: ACC = rows of B (off-diagonal); also the column-split copy of Xb for MMA3 (OB is free now)
+      // ---- E2: ACC = rows of B (off-diagonal)
       wait_mma();
+      TR();   // MMA2 done
       {
         uint32_t r[2][16];
         tmem_ld16(acc_t, r[0]);
@@ -309,17 +355,25 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           pack16(r[q & 1], p);
           if (own) set_one(p, dq == q ? dword : 8, dkeep, 0u);
           tmem_st8(opa_t + 8 * q, p);
-          uint32_t x8[8];
-#pragma unroll
-          for (int j = 0; j < 8; ++j) x8[j] = cvt_bf16x2(xs[8 * q + j]);
-          st_cluster_v4(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
-          st_cluster_v4(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
         }
       }
+      TR();   // E2 loop done
       ready_and_issue(3);
+      TR();   // MMA3 issued
 
       // ---- E3: Xh = (a + B_RR) Xh + offdiag(B) Xh
       wait_mma();
+      TR();   // MMA3 done
+      if (last && nxt < n_items) {                           // XB and OB are free (every pair MMA has completed)
+        if (lead) issue_gm(nxt);
+        prefetched = true;
+      }
+      if (last && lead && step_mode) {                       // ... and so is ST: fetch W into it
+        mbar_arrive_expect_tx(w_bar, kBufBytes);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tma_load_2d(ST + j * kBlkBytes, map_w, x0 + 64 * j, y0, w_bar);
+        w_issued = true;
+      }
       {
         const f2 si2 = pk2(si, si);
         f2 Da = pk2(0.f, 0.f), Db = Da;
@@ -352,12 +406,15 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           ctrl->dpart[q4][t] = d0 + d1;
         }
       }
+      TR();   // E3 loop done
       if (!last) {
         ready_and_issue(1);
+        write_xb_copy(xs);
         di = (ctrl->dpart[0][t] + ctrl->dpart[1][t]) + (ctrl->dpart[2][t] + ctrl->dpart[3][t]);
       } else {
         tc_fence_before_sync();
       }
+      TR();   // MMA1 of the next step issued (or nothing)
     }
 
     // ---------------- F: untile + scaled, weight-decayed write --------------------------------
@@ -428,3 +485,9 @@ cudaError_t launch_tc256(const LaunchArgs& a, cudaStream_t s) {
 }
 
 }  // namespace himuon
+
+#ifdef HIMUON_TRACE
+extern "C" int himuon_debug_read_trace(long long* out, int n) {
+  return (int)cudaMemcpyFromSymbol(out, himuon::g_trace, sizeof(long long) * (size_t)n, 0, cudaMemcpyDeviceToHost);
+}
+#endif

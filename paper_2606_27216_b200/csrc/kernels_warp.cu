@@ -121,6 +121,30 @@ __device__ __forceinline__ TileIO make_io(void* ptr, long long ld, int H, int W)
   return io;
 }
 
+// Interior tile with 32-bit-aligned rows: every element pair of the thread is one unchecked 32-bit access at
+// base + (2 i + rr) * rows8 + (2 j + nh) * 4 words (base = the thread's first pair, rows8 = 8 rows in words).
+struct FastTile {
+  bool ok;
+  long long g8, m8, w8;         // 8 rows of G / M / W in 32-bit words
+  const uint32_t* g;
+  uint32_t* m;
+  uint32_t* w;
+};
+__device__ __forceinline__ FastTile make_fast(const LayerDev& L, int row0, int col0, int T, int g, int c, bool step_mode) {
+  FastTile f;
+  const uintptr_t al = reinterpret_cast<uintptr_t>(L.g) | reinterpret_cast<uintptr_t>(L.w) |
+                       (step_mode ? reinterpret_cast<uintptr_t>(L.m) : 0);
+  f.ok = (row0 + T <= L.H) && (col0 + T <= L.W) && ((al & 3) == 0) && (((L.ld_g | L.ld_w | (step_mode ? L.ld_m : 0)) & 1) == 0);
+  const long long r = row0 + g, cc = col0 + 2 * c;
+  f.g = reinterpret_cast<const uint32_t*>(reinterpret_cast<const __nv_bfloat16*>(L.g) + r * L.ld_g + cc);
+  f.m = reinterpret_cast<uint32_t*>(reinterpret_cast<__nv_bfloat16*>(L.m) + r * L.ld_m + cc);
+  f.w = reinterpret_cast<uint32_t*>(reinterpret_cast<__nv_bfloat16*>(L.w) + r * L.ld_w + cc);
+  f.g8 = 4 * L.ld_g;
+  f.m8 = 4 * L.ld_m;
+  f.w8 = 4 * L.ld_w;
+  return f;
+}
+
 // The K Newton-Schulz steps on one tile held in registers.  SPLIT: the bf16 operand made from the fp32
 // iterate is complemented by the bf16 rounding of its remainder (Gram product with 3 MMAs, B X with 2).
 template <int NB, bool SPLIT>
@@ -276,6 +300,16 @@ himuon_warp_kernel(const LayerDev* __restrict__ layers, const WorkItem* __restri
     L = layers[wi.layer];
     row0 = wi.r * T;
     col0 = wi.c * T;
+    const FastTile ft = make_fast(L, row0, col0, T, g, c, step_mode);
+    if (ft.ok) {
+#pragma unroll
+      for (int q = 0; q < NB * NB * 4; ++q) {
+        const int i2 = q / (NB * 4), j2 = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
+        gq[q] = __ldg(ft.g + (2 * i2 + rr) * ft.g8 + (2 * j2 + nh) * 4);
+        mq[q] = step_mode ? ft.m[(2 * i2 + rr) * ft.m8 + (2 * j2 + nh) * 4] : 0u;
+      }
+      return;
+    }
     const TileIO ioG = make_io(L.g, L.ld_g, L.H, L.W);
     const TileIO ioM = make_io(L.m, L.ld_m, L.H, L.W);
 #pragma unroll
@@ -298,6 +332,7 @@ himuon_warp_kernel(const LayerDev* __restrict__ layers, const WorkItem* __restri
     const int row0 = rown, col0 = coln;
     const TileIO ioM = make_io(L.m, L.ld_m, L.H, L.W);
     const TileIO ioW = make_io(L.w, L.ld_w, L.H, L.W);
+    const FastTile ft = make_fast(L, row0, col0, T, g, c, step_mode);
 
     // ---------------- P: momentum, Frobenius normalisation ----------
     Blk x[NB][NB];
@@ -311,8 +346,9 @@ himuon_warp_kernel(const LayerDev* __restrict__ layers, const WorkItem* __restri
       if (step_mode) {
         const float m0 = fmaf(hp.beta, __uint_as_float(mq[q] << 16), g0);
         const float m1 = fmaf(hp.beta, __uint_as_float(mq[q] & 0xffff0000u), g1);
-        ioM.store2(row, col, m0, m1);
-        h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;
+        if (ft.ok) ft.m[(2 * i + rr) * ft.m8 + (2 * j + nh) * 4] = pack2(m0, m1);
+        else ioM.store2(row, col, m0, m1);
+        h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;     // Ghat = G + beta M' (Nesterov) | M'
         h1 = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
       }
       x[i][j].v[nh][2 * rr] = h0;
@@ -325,7 +361,9 @@ himuon_warp_kernel(const LayerDev* __restrict__ layers, const WorkItem* __restri
 #pragma unroll
     for (int q = 0; q < NB * NB * 4; ++q) {
       const int i = q / (NB * 4), j = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
-      wq[q] = step_mode ? ioW.load2_raw(row0 + 16 * i + g + 8 * rr, col0 + 16 * j + 8 * nh + 2 * c) : 0u;
+      if (!step_mode) wq[q] = 0u;
+      else if (ft.ok) wq[q] = ft.w[(2 * i + rr) * ft.w8 + (2 * j + nh) * 4];
+      else wq[q] = ioW.load2_raw(row0 + 16 * i + g + 8 * rr, col0 + 16 * j + 8 * nh + 2 * c);
     }
     float tot = ss;
 #pragma unroll
@@ -370,7 +408,8 @@ himuon_warp_kernel(const LayerDev* __restrict__ layers, const WorkItem* __restri
         o0 = fmaf(keep, __uint_as_float(wq[q] << 16), o0);
         o1 = fmaf(keep, __uint_as_float(wq[q] & 0xffff0000u), o1);
       }
-      ioW.store2(row, col, o0, o1);
+      if (ft.ok) ft.w[(2 * i + rr) * ft.w8 + (2 * j + nh) * 4] = pack2(o0, o1);
+      else ioW.store2(row, col, o0, o1);
     }
     it = nx;
   }

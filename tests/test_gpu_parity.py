@@ -205,18 +205,20 @@ def test_tc128_step(nesterov, wd):
         assert torch.equal(Gd[i].cpu(), Gs[i])
 
 
-def test_tc128_chunked_equals_unchunked():
-    """Memory-bounded chunking is mathematically equivalent: >= 3 chunks, bit-identical."""
+@pytest.mark.parametrize("T", [128, 16, 32, 64, 256])
+def test_chunked_equals_unchunked(T):
+    """Memory-bounded chunking is mathematically equivalent: >= 3 chunks, bit-identical,
+    for every bf16 kernel path (T = 64 pairs tiles across chunk boundaries differently: still bit-identical)."""
     _need_gpu()
-    shapes = [(256, 384), (384, 256), (128, 128)]
+    shapes = [(2 * T, 3 * T), (3 * T, 2 * T), (T, T + T // 2)]
     Ws, Gs, Ms = _param_set(shapes, 25)
     hp = hm.HParams(K=5, eps=1e-7, wd=0.01)
     outs = []
-    probe = hm.Plan.from_tensors(Ws, Gs, Ms, 128)
+    probe = hm.Plan.from_tensors(Ws, Gs, Ms, T)
     fixed = probe.workspace_bytes - 16 * probe.n_tiles
     for cap in (0, fixed + 16 * 5):
         Wd, Gd, Md = [w.to(DEV) for w in Ws], [g.to(DEV) for g in Gs], [m.to(DEV) for m in Ms]
-        plan = hm.Plan.from_tensors(Wd, Gd, Md, 128, workspace_cap_bytes=cap).bind()
+        plan = hm.Plan.from_tensors(Wd, Gd, Md, T, workspace_cap_bytes=cap).bind()
         if cap:
             assert plan.n_chunks >= 3
         plan.step(hp)
@@ -226,7 +228,9 @@ def test_tc128_chunked_equals_unchunked():
         assert torch.equal(outs[0][0][i], outs[1][0][i]) and torch.equal(outs[0][1][i], outs[1][1][i])
 
 
-@pytest.mark.parametrize("path,T,dtype", [(hm.HIMUON_PATH_AUTO, 128, torch.bfloat16), (hm.HIMUON_PATH_FP32, 32, torch.float32)])
+@pytest.mark.parametrize("path,T,dtype", [(hm.HIMUON_PATH_AUTO, 128, torch.bfloat16), (hm.HIMUON_PATH_FP32, 32, torch.float32),
+                                          (hm.HIMUON_PATH_AUTO, 16, torch.bfloat16), (hm.HIMUON_PATH_AUTO, 32, torch.bfloat16),
+                                          (hm.HIMUON_PATH_AUTO, 64, torch.bfloat16), (hm.HIMUON_PATH_AUTO, 256, torch.bfloat16)])
 def test_indexing_bit_exact(path, T, dtype):
     """Tile indexing / reassembly with integer-tagged inputs, bit-exact (BASELINE north_star):
     lr = 0 leaves W bitwise unchanged; beta = 0 makes M' == G bitwise; gutters untouched."""

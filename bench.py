@@ -274,7 +274,9 @@ def run_gpu(args):
 
 def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
     """Per step: H2D copy of the step's gradients from pinned host memory, himuon_step, D2H read of the
-    updated weights into pinned host memory.  Host buffers are bounded by --e2e-host-gb."""
+    updated weights into pinned host memory - through the public API (one bound plan per group of layers),
+    pipelined over three streams so that the copies of one group overlap the step of another (PCIe is full
+    duplex).  Host buffers are bounded by --e2e-host-gb."""
     sizes = [g.numel() * 2 for g in Gs]
     budget = int(args.e2e_host_gb * (1 << 30))
     n_layers, acc = 0, 0
@@ -285,34 +287,60 @@ def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
         n_layers += 1
     n_layers = max(n_layers, 1)
     full = n_layers == len(Gs)
-    sub_Ws, sub_Gs = Ws[:n_layers], Gs[:n_layers]
-    if full:
-        sub_plan, sub_flops = plan, flops
-    else:
-        Ms_sub = [torch.zeros_like(g) for g in sub_Gs]
-        Tl = [l.T for l in spec.layers[:n_layers]]
-        sub_plan = hm.Plan.from_tensors(sub_Ws, sub_Gs, Ms_sub, args.T, T_per_layer=Tl if any(Tl) else None).bind()
-        sub_flops = float(sum(6.0 * args.K * (l.T or args.T) * l.H * l.W for l in spec.layers[:n_layers]))
-    hG = [torch.empty(g.shape, dtype=g.dtype, pin_memory=True) for g in sub_Gs]
-    hW = [torch.empty(w.shape, dtype=w.dtype, pin_memory=True) for w in sub_Ws]
-    for h, g in zip(hG, sub_Gs):
-        h.copy_(g)
+    per_group = max(1, {"gpt2": 6}.get(spec.name[:4], 7))
+    groups = [list(range(a, min(a + per_group, n_layers))) for a in range(0, n_layers, per_group)]
+    Tl = [l.T for l in spec.layers]
+    plans = []
+    for gr in groups:
+        Ms_g = [torch.zeros_like(Gs[i]) for i in gr]
+        plans.append(hm.Plan.from_tensors([Ws[i] for i in gr], [Gs[i] for i in gr], Ms_g, args.T,
+                                          T_per_layer=[Tl[i] for i in gr] if any(Tl) else None).bind())
+    sub_flops = float(sum(6.0 * args.K * (spec.layers[i].T or args.T) * spec.layers[i].H * spec.layers[i].W for i in range(n_layers)))
+    hG = [torch.empty(Gs[i].shape, dtype=Gs[i].dtype, pin_memory=True) for i in range(n_layers)]
+    hW = [torch.empty(Ws[i].shape, dtype=Ws[i].dtype, pin_memory=True) for i in range(n_layers)]
+    for i in range(n_layers):
+        hG[i].copy_(Gs[i])
     steps = max(2, min(args.steps, 5))
+    s_in, s_cmp, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    ev_cmp_prev = [None] * len(groups)       # G of a group may be overwritten once the previous step of it is done
+    ev_out_prev = [None] * len(groups)       # W of a group may be overwritten once its previous read-back is done
 
     def one():
-        for h, g in zip(hG, sub_Gs):
-            g.copy_(h, non_blocking=True)
-        sub_plan.step(hp)
-        for h, w in zip(hW, sub_Ws):
-            h.copy_(w, non_blocking=True)
+        for k, gr in enumerate(groups):
+            with torch.cuda.stream(s_in):
+                if ev_cmp_prev[k] is not None:
+                    s_in.wait_event(ev_cmp_prev[k])
+                for i in gr:
+                    Gs[i].copy_(hG[i], non_blocking=True)
+                e_in = torch.cuda.Event(); e_in.record(s_in)
+            with torch.cuda.stream(s_cmp):
+                s_cmp.wait_event(e_in)
+                if ev_out_prev[k] is not None:
+                    s_cmp.wait_event(ev_out_prev[k])
+                plans[k].step(hp, stream=s_cmp)
+                e_c = torch.cuda.Event(); e_c.record(s_cmp)
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(e_c)
+                for i in gr:
+                    hW[i].copy_(Ws[i], non_blocking=True)
+                e_o = torch.cuda.Event(); e_o.record(s_out)
+            ev_cmp_prev[k], ev_out_prev[k] = e_c, e_o
 
-    one()
+    def join(stream):
+        for s_ in (s_in, s_cmp, s_out):
+            e = torch.cuda.Event(); e.record(s_); stream.wait_event(e)
+
+    cur = torch.cuda.current_stream()
+    one(); join(cur)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    e0.record(cur)
+    for s_ in (s_in, s_cmp, s_out):
+        s_.wait_event(e0)
     for _ in range(steps):
         one()
-    e1.record()
+    join(cur)
+    e1.record(cur)
     barrier()
     ms = e0.elapsed_time(e1) / steps
     if world > 1:
@@ -324,6 +352,7 @@ def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
     d2h = sum(h.numel() * 2 for h in hW)
     return {"value": round(world * sub_flops / (ms * 1e-3) / 1e12, 3), "unit": UNIT, "ms_per_step": round(ms, 3),
             "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": steps,
+            "pipeline": f"{len(groups)} groups of layers (one plan each) over 3 streams: H2D | himuon_step | D2H",
             "workload": "full parameter set" if full else f"first {n_layers} of {len(Gs)} layers (host-buffer budget {args.e2e_host_gb} GB)"}
 
 

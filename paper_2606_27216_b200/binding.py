@@ -167,7 +167,7 @@ class HParams:
 
 def himuon_supported_tile_sizes(dtype_code: int, path: int = HIMUON_PATH_AUTO) -> List[int]:
     mask = _lib().himuon_supported_tile_sizes(dtype_code, path)
-    return [16 << i for i in range(5) if mask & (1 << i)]
+    return [16 << i for i in range(16) if mask & (1 << i)]
 
 
 def himuon_launch_count() -> int:

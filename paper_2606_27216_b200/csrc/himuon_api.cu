@@ -23,7 +23,7 @@ himuon_status cuda_fail(cudaError_t e, const char* what) {
 
 constexpr size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-const int kTileSizes[] = {16, 32, 64, 128, 256};
+const int kTileSizes[] = {16, 32, 64, 128, 256, 512};
 
 // Which kernel serves (dtype, requested path, T); -1 = none in this build.
 // W = number of columns of the matrix (0 = unknown / any).  The TMA stores of the tensor-core path
@@ -32,10 +32,12 @@ const int kTileSizes[] = {16, 32, 64, 128, 256};
 // of the last granule, i.e. it would write into the ld - W gutter).
 int select_kpath(int dtype, int path, int T, int W = 0) {
   const bool simt_ok = (T == 16 || T == 32 || T == 64 || T == 128);
-  if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : -1;
-  // bf16 storage, AUTO: tensor-core path where it exists, else the fp32 kernel.
+  if (T >= 512) return KPATH_GEMM;                                  // library-size products: cuBLAS
+  if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : (T == 256 ? KPATH_GEMM : -1);
+  // bf16 storage, AUTO: tensor-core path where it exists, else the fp32 kernel / the large-tile path.
   if ((T == 256 || T == 128 || T == 64) && (W % 8) == 0) return KPATH_TC;
   if (T == 16 || T == 32) return KPATH_WARP;
+  if (T == 256) return KPATH_GEMM;                                  // width not a multiple of 8
   return simt_ok ? KPATH_FP32_SIMT : -1;
 }
 
@@ -153,7 +155,7 @@ int64_t himuon_launch_count(void) { return g_launches.load(); }
 
 int32_t himuon_supported_tile_sizes(int32_t dtype, int32_t path) {
   int32_t mask = 0;
-  for (int i = 0; i < 5; ++i)
+  for (int i = 0; i < (int)(sizeof(kTileSizes) / sizeof(kTileSizes[0])); ++i)
     if (select_kpath(dtype, path, kTileSizes[i]) >= 0) mask |= (1 << i);
   return mask;
 }
@@ -204,7 +206,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
     int Te;
     if (full) {
       Te = smallest_supported_T_at_least(mx, dt, path);
-      if (Te < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
+      if (Te < 0) Te = kWholeMatrixT;          // larger than every tile size: one whole-matrix item on the cuBLAS path
     } else {
       bool known = false;
       for (int t : kTileSizes) known |= (t == T);
@@ -213,7 +215,11 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       Te = T;
     }
     const int kp = select_kpath(dt, path, Te, W);
-    if (kp < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }   // e.g. T = 256 on a bf16 width that is not a multiple of 8
+    if (kp < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
+    if (kp == KPATH_GEMM) {
+      const size_t need = gemm_path_scratch_bytes(H < Te ? H : Te, W < Te ? W : Te);
+      if (need > p->scratch_bytes) p->scratch_bytes = need;
+    }
     p->T_eff[l] = Te;
     p->kpath[l] = kp;
     if (!L.g.ptr || !L.w.ptr) p->bindable = false;
@@ -259,7 +265,8 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
 
   // Workspace layout: [layer table][tensor maps][work items of the resident list / current chunk].
   p->off_tmaps   = align_up((size_t)n_layers * sizeof(LayerDev), 128);
-  p->off_items   = p->off_tmaps + (p->needs_tma ? (size_t)n_layers * 3 * sizeof(CUtensorMap) : 0);
+  p->off_scratch = align_up(p->off_tmaps + (p->needs_tma ? (size_t)n_layers * 3 * sizeof(CUtensorMap) : 0), 256);
+  p->off_items   = p->off_scratch + p->scratch_bytes;
   p->fixed_bytes = p->off_items;
   const long long n_total = (long long)p->items.size();
   std::vector<long long> offs;
@@ -377,6 +384,14 @@ static himuon_status run_plan(himuon_plan* plan, const himuon_hparams* hp, int m
   for (const Chunk& c : plan->chunks) {
     if (c.end == c.begin) continue;
     const Bucket& B = plan->buckets[c.bucket];
+    if (B.kpath == KPATH_GEMM) {   // large tiles: the items are walked on the host, products go to cuBLAS
+      long long   n_launch = 0;
+      cudaError_t e = run_gemm_path(plan->layer_dev.data(), plan->items.data() + c.begin, c.end - c.begin, B.T, mode,
+                                    B.dtype, *hp, ws + plan->off_scratch, s, &n_launch);
+      g_launches.fetch_add(n_launch);
+      if (e != cudaSuccess) return cuda_fail(e, "step: large-tile path (cuBLAS)");
+      continue;
+    }
     LaunchArgs    a;
     a.layers = (const LayerDev*)ws;
     a.tmaps  = plan->needs_tma ? (const CUtensorMap*)(ws + plan->off_tmaps) : nullptr;
@@ -407,7 +422,9 @@ himuon_status himuon_phi(himuon_plan* plan, const himuon_hparams* hp, void* cuda
   return run_plan(plan, hp, MODE_PHI, cuda_stream);
 }
 
-size_t himuon_ns_tiles_workspace_bytes(void) { return 128 + 3 * sizeof(CUtensorMap); }
+size_t himuon_ns_tiles_workspace_bytes(void) {
+  return align_up(128 + 3 * sizeof(CUtensorMap), 256) + gemm_path_scratch_bytes(512, 512);
+}
 
 himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_tiles, int32_t T,
                               int32_t dtype, int32_t path, int32_t K, float a, float b, float c,
@@ -440,6 +457,16 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
   D.w = tiles_out; D.g = const_cast<void*>(tiles_in); D.m = nullptr;
   D.ld_w = T; D.ld_g = T; D.ld_m = 0;
   D.H = (int)(n_tiles * T); D.W = T; D.tau_base = 0.f; D.dtype = dtype;
+  if (kp == KPATH_GEMM) {   // large tiles: host walk, cuBLAS products (scratch behind the table area of the workspace)
+    std::vector<WorkItem> its((size_t)n_tiles);
+    for (int64_t i = 0; i < n_tiles; ++i) its[(size_t)i] = WorkItem{0, (int)i, 0, 0};
+    long long   n_launch = 0;
+    cudaError_t eg = run_gemm_path(&D, its.data(), n_tiles, T, MODE_PHI, dtype, hp,
+                                   ws + align_up(128 + 3 * sizeof(CUtensorMap), 256), s, &n_launch);
+    g_launches.fetch_add(n_launch);
+    if (eg != cudaSuccess) return cuda_fail(eg, "ns_tiles: large-tile path (cuBLAS)");
+    return HIMUON_OK;
+  }
   cudaError_t e = cudaMemcpyAsync(ws, &D, sizeof(D), cudaMemcpyHostToDevice, s);
   if (e != cudaSuccess) return cuda_fail(e, "ns_tiles: layer table");
   if (kp == KPATH_TC) {

@@ -34,7 +34,8 @@ struct WorkItem {
 static_assert(sizeof(WorkItem) == 16, "WorkItem must be 16 bytes");
 
 enum Mode : int { MODE_STEP = 0, MODE_PHI = 1 };
-enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1, KPATH_WARP = 2 };
+enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1, KPATH_WARP = 2, KPATH_GEMM = 3 };
+constexpr int kWholeMatrixT = 1 << 20;   // tile size of the full-matrix branch beyond the largest tile kernel (R = C = 1)
 
 struct LaunchArgs {
   const LayerDev*    layers;     // device
@@ -57,6 +58,11 @@ cudaError_t launch_tc64(const LaunchArgs& a, cudaStream_t stream);
 cudaError_t launch_tc256(const LaunchArgs& a, cudaStream_t stream);
 // kernels_warp.cu -- mma.sync bf16 path, one warp per tile, T in {16, 32}, bf16 storage.
 cudaError_t launch_warp(const LaunchArgs& a, cudaStream_t stream);
+
+// kernels_gemm.cu -- large tiles (T = 512, full-matrix branch beyond 256): cuBLAS products, host walk over the items.
+size_t      gemm_path_scratch_bytes(int h, int w);
+cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_host, long long n_items, int T, int mode,
+                          int dtype, const himuon_hparams& hp, void* scratch, cudaStream_t stream, long long* launches);
 
 int  device_sm_count();
 void note_launch();
@@ -89,7 +95,8 @@ struct himuon_plan {
   bool      bindable  = true;                // all pointers non-null
   bool      needs_tma = false;
   size_t    fixed_bytes = 0;                 // layer table + tensor maps
-  size_t    off_tmaps = 0, off_items = 0;
+  size_t    off_tmaps = 0, off_items = 0, off_scratch = 0;
+  size_t    scratch_bytes = 0;               // large-tile path only
   long long max_chunk_tiles = 0;
   size_t    workspace_bytes = 0;
   size_t    cap = 0;

@@ -1,0 +1,82 @@
+"""GPU parity tests of the large-tile path (csrc/kernels_gemm.cu): T = 512 tiles and the full-matrix branch
+T >= max(H, W) beyond 256 (the paper's T = infinity warm start and its T = 512 default, PAPER.md:135-138, :243-249,
+:386), whose products run on cuBLAS.  Tolerances: bf16 storage (TF32 products) 3e-2, fp32 storage 1e-4."""
+import numpy as np
+import pytest
+import torch
+
+import himuon_inputs as I
+import paper_2606_27216_b200 as hm
+import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+
+
+def _run_phi(G, T, hp, path=hm.HIMUON_PATH_AUTO):
+    Gd = G.to(DEV)
+    Ud = torch.full_like(Gd, float("nan"))
+    plan = hm.Plan.from_tensors([Ud], [Gd], None, T, path=path).bind()
+    plan.phi(hp)
+    torch.cuda.synchronize()
+    plan.destroy()
+    return Ud.cpu()
+
+
+@pytest.mark.parametrize("H,W,T", [(1024, 1536, 512), (700, 520, 512), (640, 384, 100000), (300, 900, 1024), (512, 512, 512)])
+def test_large_tiles_phi_bf16(H, W, T):
+    _need_gpu()
+    G = I.lowrank_plus_noise(H, W, 32, seed_cfg=71, layer_index=0, tensor_id=I.TENSOR_G)
+    hp = hm.HParams(K=5, eps=1e-7)
+    U = _run_phi(G, T, hp)
+    PU.check_phi(U, G, T, hp, PU.TOL_TC, out_is_bf16=True)
+
+
+@pytest.mark.parametrize("H,W,T", [(600, 400, 1024), (512, 768, 256), (520, 1030, 512)])
+def test_large_tiles_phi_fp32(H, W, T):
+    """fp32 storage: true fp32 products, the <= 1e-4 path (also T = 256 on fp32 storage)."""
+    _need_gpu()
+    G = I.gaussian(H, W, seed_cfg=72, dtype=torch.float32)
+    hp = hm.HParams(K=5, eps=1e-7)
+    U = _run_phi(G, T, hp)
+    PU.check_phi(U, G, T, hp, PU.TOL_FP32, out_is_bf16=False)
+
+
+@pytest.mark.parametrize("nesterov", [True, False])
+def test_full_to_local_schedule_step(nesterov):
+    """One step each of the paper's schedule infinity -> 512 -> 128 on the same parameters; momentum buffers are
+    plan-independent and survive re-planning."""
+    _need_gpu()
+    shapes = [(768, 1024), (1024, 520)]
+    Ws, Gs, Ms = [], [], []
+    for i, (h, w) in enumerate(shapes):
+        Gs.append(I.lowrank_plus_noise(h, w, 32, seed_cfg=73, layer_index=i, tensor_id=I.TENSOR_G))
+        Ms.append(I.lowrank_plus_noise(h, w, 32, seed_cfg=73, layer_index=i, tensor_id=I.TENSOR_M))
+        Ws.append(I.gaussian(h, w, seed_cfg=73, layer_index=i, tensor_id=I.TENSOR_W, dtype=torch.bfloat16, scale=0.02))
+    hp = hm.HParams(K=5, eps=1e-7, beta=0.95, nesterov=nesterov, lr=0.02, wd=0.01, scale_c=0.2)
+    Wd, Gd, Md = [w.to(DEV) for w in Ws], [g.to(DEV) for g in Gs], [m.to(DEV) for m in Ms]
+    Wh, Mh = [w.clone() for w in Ws], [m.clone() for m in Ms]
+    for T in (1 << 20, 512, 128):
+        plan = hm.Plan.from_tensors(Wd, Gd, Md, T).bind()
+        plan.step(hp)
+        torch.cuda.synchronize()
+        plan.destroy()
+        for i in range(len(shapes)):
+            PU.check_step(Wh[i], Gs[i], Mh[i], Wd[i].cpu(), Md[i].cpu(), T, hp, PU.TOL_TC, storage_bf16=True)
+            Wh[i], Mh[i] = Wd[i].cpu(), Md[i].cpu()          # continue from what the GPU stored
+
+
+def test_ns_tiles_512():
+    _need_gpu()
+    tiles = torch.stack([I.row_scaled_gaussian(512, 512, seed_cfg=74 + i, dtype=torch.bfloat16) for i in range(2)])
+    out = hm.himuon_ns_tiles(tiles.to(DEV), K=5, eps=1e-7).cpu()
+    ohp = PU.oracle_hp(hm.HParams(K=5, eps=1e-7))
+    for i in range(2):
+        ref = PU.O.phi(PU.f64(tiles[i]), ohp.K, ohp.a, ohp.b, ohp.c, ohp.eps)
+        e = np.linalg.norm(PU.f64(out[i]) - ref) / np.linalg.norm(ref)
+        assert e <= PU.TOL_TC, f"tile {i}: {e:.3e}"

@@ -131,9 +131,9 @@ def test_full_branch_is_one_padded_tile():
     assert lrc.tolist() == [[0, 0, 0]] and cT.tolist() == [128]
     p = hm.Plan(_layers([(20, 30)], hm.HIMUON_F32), 128)
     assert p.worklist()[2].tolist() == [32]
-    with pytest.raises(hm.HimuonError) as e:
-        hm.Plan(_layers([(4096, 4096)]), 8192)
-    assert e.value.status == B.HIMUON_ERR_UNSUPPORTED
+    # larger than every tile kernel: one whole-matrix item on the large-tile (cuBLAS) path
+    p = hm.Plan(_layers([(4096, 4096)]), 8192)
+    assert p.n_tiles == 1 and p.workspace_bytes > 2 * 4096 * 4096 * 4
 
 
 def test_argument_validation():
@@ -171,17 +171,21 @@ def test_tma_alignment_is_checked():
 
 
 def test_supported_tile_sizes_per_dtype_and_path():
-    assert hm.himuon_supported_tile_sizes(hm.HIMUON_F32) == [16, 32, 64, 128]
-    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16) == [16, 32, 64, 128, 256]
-    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16, hm.HIMUON_PATH_FP32) == [16, 32, 64, 128]
-    with pytest.raises(hm.HimuonError) as e:
-        hm.Plan(_layers([(512, 512)], hm.HIMUON_F32), 256)      # no fp32 kernel for T = 256
-    assert e.value.status == B.HIMUON_ERR_UNSUPPORTED
-    with pytest.raises(hm.HimuonError) as e:
-        hm.Plan(_layers([(512, 300)]), 256)                     # bf16 T = 256 needs a width that is a multiple of 8
-    assert e.value.status == B.HIMUON_ERR_UNSUPPORTED
-    assert hm.Plan(_layers([(512, 512)]), 256).n_tiles == 4
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_F32) == [16, 32, 64, 128, 256, 512]
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16) == [16, 32, 64, 128, 256, 512]
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16, hm.HIMUON_PATH_FP32) == [16, 32, 64, 128, 256, 512]
+    # T = 256 without a tile kernel (fp32 storage; bf16 width not a multiple of 8) and T = 512 run on the
+    # large-tile path, whose scratch is part of the plan's workspace
+    small = hm.Plan(_layers([(512, 512)]), 256)
+    assert small.n_tiles == 4 and small.workspace_bytes < 1 << 20
+    for pl in (hm.Plan(_layers([(512, 512)], hm.HIMUON_F32), 256), hm.Plan(_layers([(512, 304), (512, 300)]), 256)):
+        assert pl.workspace_bytes > 32 << 20
+    p = hm.Plan(_layers([(1024, 1536)]), 512)
+    assert p.n_tiles == 6 and p.workspace_bytes > (32 << 20) + 2 * 512 * 512 * 4
     assert hm.Plan(_layers([(200, 256)]), 256).n_tiles == 1     # full-matrix branch served by the T = 256 kernel
+    with pytest.raises(hm.HimuonError) as e:                    # the scratch counts against the workspace cap
+        hm.Plan(_layers([(4096, 4096)]), 8192, workspace_cap_bytes=64 << 20)
+    assert e.value.status == B.HIMUON_ERR_WORKSPACE_TOO_SMALL
 
 
 def test_kernel_paths_bucket_the_work_list():

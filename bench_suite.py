@@ -48,7 +48,8 @@ def _step_rows(args, hm, pk, dev):
     from bench import spec_of, algorithmic_flops, make_inputs
     hp = hm.HParams(K=args.K, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
     for name, T, cap in (("gpt2-small", 128, 2048), ("gpt2-xl", 128, 256), ("llama3-8b", 128, 2048),
-                         ("llama3-8b", 64, 2048), ("llama3-8b-sched", 128, 2048)):
+                         ("llama3-8b", 64, 2048), ("llama3-8b", 256, 2048), ("llama3-8b-sched", 128, 2048),
+                         ("llama3-8b", 512, 2048), ("llama3-8b", 1 << 20, 2048)):
         spec = spec_of(name)
         row = {"row": "step", "workload": name, "T": T, "cap_mb": cap}
         try:
@@ -57,8 +58,9 @@ def _step_rows(args, hm, pk, dev):
             Tl = [l.T for l in spec.layers]
             plans = [hm.Plan.from_tensors(W, G, M, T, T_per_layer=Tl if any(Tl) else None,
                                           workspace_cap_bytes=cap << 20).bind() for (W, G, M) in sets]
-            flops = algorithmic_flops(spec, T, args.K)
-            med, best = _time(lambda i: plans[i % n_sets].step(hp), args.steps)
+            flops = algorithmic_flops(spec, T, args.K) if T <= 512 else float(sum(
+                6.0 * args.K * min(l.H, l.W) * l.H * l.W for l in spec.layers))   # full matrix: Gram on the short side
+            med, best = _time(lambda i: plans[i % n_sets].step(hp), args.steps if T <= 256 else 2)
             bound, roof_ms = _roof(flops, 10.0 * spec.n_elements, pk)
             row.update({"ms": round(med, 4), "ms_min": round(best, 4), "tflops": round(flops / med / 1e9, 2),
                         "gbs": round(10.0 * spec.n_elements / med / 1e6, 1), "bound": bound,
@@ -92,7 +94,7 @@ def _sweep_rows(args, hm, pk, dev):
         n_sets = max(1, -(-2 * L2_BYTES // (4 * H * W)))
         Gs = [I.row_scaled_gaussian(H, W, seed_cfg=2, layer_index=i, dtype=torch.bfloat16, device=dev) for i in range(n_sets)]
         Us = [torch.empty_like(g) for g in Gs]
-        for T in (16, 32, 64, 128, 256):
+        for T in (16, 32, 64, 128, 256, 512):
             row = {"row": "phi_sweep", "workload": f"{H}x{W} bf16 row-scaled gaussian (config 3)", "T": T}
             try:
                 plans = [hm.Plan.from_tensors([u], [g], None, T).bind() for u, g in zip(Us, Gs)]

@@ -2,6 +2,7 @@
 // chunking -- PAPER.md:231-241, sec. 4.4.2-4.4.3), binding of the plan's device tables, and dispatch
 // of one kernel launch per chunk.  See include/himuon.h for the contract of every entry point.
 #include <atomic>
+#include <map>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -192,6 +193,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
   p->layer_dev.resize(n_layers);
 
   himuon_status st = HIMUON_OK;
+  std::map<int, long long> gemm_tiles;   // large-tile path: tiles per tile size so far
   for (int l = 0; l < n_layers && st == HIMUON_OK; ++l) {
     const himuon_layer& L = layers[l];
     const int H = L.g.H, W = L.g.W, dt = L.g.dtype;
@@ -217,7 +219,19 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
     const int kp = select_kpath(dt, path, Te, W);
     if (kp < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
     if (kp == KPATH_GEMM) {
-      const size_t need = gemm_path_scratch_bytes(H < Te ? H : Te, W < Te ? W : Te);
+      size_t need;
+      if (Te <= 512) {   // uniform tiles run in sub-batches: as many tiles as a scratch budget holds (>= 1)
+        const size_t per = gemm_path_batch_item_bytes(Te);
+        size_t       budget = (size_t)512 << 20;
+        if (workspace_cap_bytes && workspace_cap_bytes / 2 < budget) budget = workspace_cap_bytes / 2;
+        gemm_tiles[Te] += (long long)((H + Te - 1) / Te) * ((W + Te - 1) / Te);
+        long long nb = (long long)(budget / per);
+        if (nb > gemm_tiles[Te]) nb = gemm_tiles[Te];
+        if (nb < 1) nb = 1;
+        need = gemm_path_fixed_bytes() + (size_t)nb * per;
+      } else {
+        need = gemm_path_scratch_bytes(H, W);
+      }
       if (need > p->scratch_bytes) p->scratch_bytes = need;
     }
     p->T_eff[l] = Te;
@@ -384,14 +398,6 @@ static himuon_status run_plan(himuon_plan* plan, const himuon_hparams* hp, int m
   for (const Chunk& c : plan->chunks) {
     if (c.end == c.begin) continue;
     const Bucket& B = plan->buckets[c.bucket];
-    if (B.kpath == KPATH_GEMM) {   // large tiles: the items are walked on the host, products go to cuBLAS
-      long long   n_launch = 0;
-      cudaError_t e = run_gemm_path(plan->layer_dev.data(), plan->items.data() + c.begin, c.end - c.begin, B.T, mode,
-                                    B.dtype, *hp, ws + plan->off_scratch, s, &n_launch);
-      g_launches.fetch_add(n_launch);
-      if (e != cudaSuccess) return cuda_fail(e, "step: large-tile path (cuBLAS)");
-      continue;
-    }
     LaunchArgs    a;
     a.layers = (const LayerDev*)ws;
     a.tmaps  = plan->needs_tma ? (const CUtensorMap*)(ws + plan->off_tmaps) : nullptr;
@@ -402,6 +408,15 @@ static himuon_status run_plan(himuon_plan* plan, const himuon_hparams* hp, int m
                                       (size_t)(c.end - c.begin) * sizeof(WorkItem), cudaMemcpyHostToDevice, s);
       if (e != cudaSuccess) return cuda_fail(e, "step: chunk work list");
       a.items = (const WorkItem*)(ws + plan->off_items);
+    }
+    if (B.kpath == KPATH_GEMM) {   // large tiles: products go to cuBLAS (sub-batches of tiles / whole matrices)
+      long long   n_launch = 0;
+      cudaError_t e = run_gemm_path(plan->layer_dev.data(), plan->items.data() + c.begin, a.layers, a.items,
+                                    c.end - c.begin, B.T, mode, B.dtype, *hp, ws + plan->off_scratch,
+                                    plan->scratch_bytes, s, &n_launch);
+      g_launches.fetch_add(n_launch);
+      if (e != cudaSuccess) return cuda_fail(e, "step: large-tile path (cuBLAS)");
+      continue;
     }
     a.n_items = c.end - c.begin;
     a.T = B.T;
@@ -461,8 +476,11 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
     std::vector<WorkItem> its((size_t)n_tiles);
     for (int64_t i = 0; i < n_tiles; ++i) its[(size_t)i] = WorkItem{0, (int)i, 0, 0};
     long long   n_launch = 0;
-    cudaError_t eg = run_gemm_path(&D, its.data(), n_tiles, T, MODE_PHI, dtype, hp,
-                                   ws + align_up(128 + 3 * sizeof(CUtensorMap), 256), s, &n_launch);
+    cudaError_t eg = cudaMemcpyAsync(ws, &D, sizeof(D), cudaMemcpyHostToDevice, s);
+    if (eg != cudaSuccess) return cuda_fail(eg, "ns_tiles: layer table");
+    // one tile per sub-batch: an implicit work list is not available on the device, so each tile is one whole block
+    eg = run_gemm_path(&D, its.data(), (const LayerDev*)ws, nullptr, n_tiles, T, MODE_PHI, dtype, hp,
+                       ws + align_up(128 + 3 * sizeof(CUtensorMap), 256), gemm_path_scratch_bytes(512, 512), s, &n_launch);
     g_launches.fetch_add(n_launch);
     if (eg != cudaSuccess) return cuda_fail(eg, "ns_tiles: large-tile path (cuBLAS)");
     return HIMUON_OK;

@@ -60,9 +60,13 @@ cudaError_t launch_tc256(const LaunchArgs& a, cudaStream_t stream);
 cudaError_t launch_warp(const LaunchArgs& a, cudaStream_t stream);
 
 // kernels_gemm.cu -- large tiles (T = 512, full-matrix branch beyond 256): cuBLAS products, host walk over the items.
-size_t      gemm_path_scratch_bytes(int h, int w);
-cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_host, long long n_items, int T, int mode,
-                          int dtype, const himuon_hparams& hp, void* scratch, cudaStream_t stream, long long* launches);
+size_t      gemm_path_scratch_bytes(int h, int w);        // one whole h x w block at a time
+size_t      gemm_path_batch_item_bytes(int T);            // per tile of a sub-batch of uniform tiles (T <= 512)
+size_t      gemm_path_fixed_bytes();                      // cuBLAS workspace inside the scratch
+cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_host, const LayerDev* layers_dev,
+                          const WorkItem* items_dev, long long n_items, int T, int mode, int dtype,
+                          const himuon_hparams& hp, void* scratch, size_t scratch_bytes, cudaStream_t stream,
+                          long long* launches);
 
 int  device_sm_count();
 void note_launch();

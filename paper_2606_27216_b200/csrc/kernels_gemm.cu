@@ -35,6 +35,10 @@ struct Cublas {
   cublasStatus_t (*gemm_ex)(cublasHandle_t, cublasOperation_t, cublasOperation_t, int, int, int, const void*,
                             const void*, cudaDataType, int, const void*, cudaDataType, int, const void*, void*,
                             cudaDataType, int, cublasComputeType_t, cublasGemmAlgo_t) = nullptr;
+  cublasStatus_t (*gemm_batched)(cublasHandle_t, cublasOperation_t, cublasOperation_t, int, int, int, const void*,
+                                 const void*, cudaDataType, int, long long, const void*, cudaDataType, int, long long,
+                                 const void*, void*, cudaDataType, int, long long, int, cublasComputeType_t,
+                                 cublasGemmAlgo_t) = nullptr;
   cublasHandle_t handle = nullptr;
   bool ok = false;
 };
@@ -52,7 +56,8 @@ Cublas& cublas() {
     c.set_stream = reinterpret_cast<decltype(c.set_stream)>(dlsym(c.lib, "cublasSetStream_v2"));
     c.set_workspace = reinterpret_cast<decltype(c.set_workspace)>(dlsym(c.lib, "cublasSetWorkspace_v2"));
     c.gemm_ex = reinterpret_cast<decltype(c.gemm_ex)>(dlsym(c.lib, "cublasGemmEx"));
-    if (!c.create || !c.set_stream || !c.set_workspace || !c.gemm_ex) return;
+    c.gemm_batched = reinterpret_cast<decltype(c.gemm_batched)>(dlsym(c.lib, "cublasGemmStridedBatchedEx"));
+    if (!c.create || !c.set_stream || !c.set_workspace || !c.gemm_ex || !c.gemm_batched) return;
     c.ok = (c.create(&c.handle) == CUBLAS_STATUS_SUCCESS);
   });
   return c;
@@ -147,6 +152,86 @@ k_update(View<S> W, const float* __restrict__ X, int h, int w, int step_mode, fl
   }
 }
 
+// ---- batched form for uniform tiles (T = 256 / 512): grid (kTileBlocks, tiles of the sub-batch) ----------------
+// The tiles of a sub-batch are staged as dense, zero-padded T x T fp32 matrices (the
+// paper's batched buffers, here bounded by a scratch budget and refilled sub-batch by sub-batch).
+constexpr int kTileBlocks = 32;
+
+template <typename S>
+__global__ void __launch_bounds__(kEwThreads)
+k_prep_b(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, float* __restrict__ X,
+         float* __restrict__ partial, int T, int step_mode, float beta, int nesterov) {
+  const WorkItem wi = items[blockIdx.y];
+  const LayerDev L = layers[wi.layer];
+  const int row0 = wi.r * T, col0 = wi.c * T;
+  const S* G = reinterpret_cast<const S*>(L.g);
+  S* M = reinterpret_cast<S*>(L.m);
+  float* Xt = X + (long long)blockIdx.y * T * T;
+  float ss = 0.f;
+  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < T * T; i += kTileBlocks * kEwThreads) {
+    const int r = i / T, c = i - r * T;
+    float x = 0.f;
+    if (row0 + r < L.H && col0 + c < L.W) {
+      const float g = ld_elem(G + (long long)(row0 + r) * L.ld_g + col0 + c);
+      x = g;
+      if (step_mode) {
+        S* pm = M + (long long)(row0 + r) * L.ld_m + col0 + c;
+        const float m = fmaf(beta, ld_elem(pm), g);
+        st_elem(pm, m);
+        x = nesterov ? fmaf(beta, m, g) : m;
+      }
+    }
+    Xt[i] = x;
+    ss = fmaf(x, x, ss);
+  }
+  __shared__ float red[kEwThreads / 32];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = ss;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    float t = 0.f;
+#pragma unroll
+    for (int i = 0; i < kEwThreads / 32; ++i) t += red[i];
+    partial[blockIdx.y * kTileBlocks + blockIdx.x] = t;
+  }
+}
+
+__global__ void __launch_bounds__(kEwThreads)
+k_scale_b(float* __restrict__ X, const float* __restrict__ partial, int T, float eps) {
+  float tot = 0.f;
+#pragma unroll
+  for (int i = 0; i < kTileBlocks; ++i) tot += partial[blockIdx.y * kTileBlocks + i];   // same order in every thread
+  const float nrm = sqrtf(tot);
+  const float inv = nrm > 0.f ? 1.f / (nrm + eps) : 0.f;
+  float* Xt = X + (long long)blockIdx.y * T * T;
+  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < T * T; i += kTileBlocks * kEwThreads) Xt[i] *= inv;
+}
+
+__global__ void k_add_diag_b(float* __restrict__ B, int T, float a) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < T) B[(long long)blockIdx.y * T * T + (long long)i * T + i] += a;
+}
+
+template <typename S>
+__global__ void __launch_bounds__(kEwThreads)
+k_update_b(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, const float* __restrict__ X, int T,
+           int step_mode, float keep, float lr_scale) {
+  const WorkItem wi = items[blockIdx.y];
+  const LayerDev L = layers[wi.layer];
+  const int row0 = wi.r * T, col0 = wi.c * T;
+  S* W = reinterpret_cast<S*>(L.w);
+  const float* Xt = X + (long long)blockIdx.y * T * T;
+  const float stepsz = lr_scale * L.tau_base;
+  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < T * T; i += kTileBlocks * kEwThreads) {
+    const int r = i / T, c = i - r * T;
+    if (row0 + r < L.H && col0 + c < L.W) {
+      S* p = W + (long long)(row0 + r) * L.ld_w + col0 + c;
+      st_elem(p, step_mode ? fmaf(keep, ld_elem(p), stepsz * Xt[i]) : Xt[i]);
+    }
+  }
+}
+
 constexpr size_t kCublasWs = 32u << 20;
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -158,7 +243,58 @@ size_t gemm_path_scratch_bytes(int h, int w) {
   return 2 * align256((size_t)h * w * 4) + 2 * align256(r * r * 4) + align256(kEwBlocks * 4) + kCublasWs;
 }
 
+// Scratch bytes per tile of the batched form: X, X2, A, B (T x T fp32 each) and the partial sums.
+size_t gemm_path_fixed_bytes() { return kCublasWs; }
+size_t gemm_path_batch_item_bytes(int T) { return 4 * align256((size_t)T * T * 4) + align256(kTileBlocks * 4); }
+
 namespace {
+
+// One sub-batch of nb uniform T x T tiles (items_dev / layers_dev: device copies of the work items and layer table).
+template <typename S>
+cudaError_t run_batch(const LayerDev* layers_dev, const WorkItem* items_dev, int nb, int T, int mode,
+                      const himuon_hparams& hp, char* scratch, cudaStream_t s, long long* launches) {
+  Cublas& cb = cublas();
+  const size_t tb = align256((size_t)T * T * 4);
+  float* X = reinterpret_cast<float*>(scratch);
+  float* X2 = reinterpret_cast<float*>(scratch + (size_t)nb * tb);
+  float* A = reinterpret_cast<float*>(scratch + 2 * (size_t)nb * tb);
+  float* B = reinterpret_cast<float*>(scratch + 3 * (size_t)nb * tb);
+  float* partial = reinterpret_cast<float*>(scratch + 4 * (size_t)nb * tb);
+  void* cws = scratch + 4 * (size_t)nb * tb + (size_t)nb * align256(kTileBlocks * 4);
+  const bool step_mode = (mode == MODE_STEP);
+  const long long stride = (long long)(tb / 4);
+  const dim3 grid(kTileBlocks, nb);
+  k_prep_b<S><<<grid, kEwThreads, 0, s>>>(layers_dev, items_dev, X, partial, T, step_mode ? 1 : 0, hp.beta, hp.nesterov);
+  k_scale_b<<<grid, kEwThreads, 0, s>>>(X, partial, T, hp.eps);
+  *launches += 2;
+  if (hp.K > 0) {
+    if (cb.set_stream(cb.handle, s) != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
+    if (cb.set_workspace(cb.handle, cws, kCublasWs) != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
+  }
+  const cublasComputeType_t ct = sizeof(S) == 4 ? CUBLAS_COMPUTE_32F : CUBLAS_COMPUTE_32F_FAST_TF32;
+  const float one = 1.f, zero = 0.f;
+  for (int k = 0; k < hp.K; ++k) {
+    // square tiles: A = X X^T = Xc^T Xc; B = b A + c A A + a I; X <- B X, i.e. Xc_new = Xc B (column-major views)
+    cublasStatus_t st = cb.gemm_batched(cb.handle, CUBLAS_OP_T, CUBLAS_OP_N, T, T, T, &one, X, CUDA_R_32F, T, stride, X,
+                                        CUDA_R_32F, T, stride, &zero, A, CUDA_R_32F, T, stride, nb, ct, CUBLAS_GEMM_DEFAULT);
+    if (st != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
+    cudaError_t e = cudaMemcpyAsync(B, A, (size_t)nb * tb, cudaMemcpyDeviceToDevice, s);
+    if (e != cudaSuccess) return e;
+    st = cb.gemm_batched(cb.handle, CUBLAS_OP_N, CUBLAS_OP_N, T, T, T, &hp.c, A, CUDA_R_32F, T, stride, A, CUDA_R_32F, T,
+                         stride, &hp.b, B, CUDA_R_32F, T, stride, nb, ct, CUBLAS_GEMM_DEFAULT);
+    if (st != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
+    k_add_diag_b<<<dim3((T + 255) / 256, nb), 256, 0, s>>>(B, T, hp.a);
+    st = cb.gemm_batched(cb.handle, CUBLAS_OP_N, CUBLAS_OP_N, T, T, T, &one, X, CUDA_R_32F, T, stride, B, CUDA_R_32F, T,
+                         stride, &zero, X2, CUDA_R_32F, T, stride, nb, ct, CUBLAS_GEMM_DEFAULT);
+    if (st != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
+    std::swap(X, X2);
+    *launches += 5;
+  }
+  k_update_b<S><<<grid, kEwThreads, 0, s>>>(layers_dev, items_dev, X, T, step_mode ? 1 : 0, 1.f - hp.lr * hp.wd,
+                                            -hp.lr * hp.scale_c);
+  *launches += 1;
+  return cudaGetLastError();
+}
 
 template <typename S>
 cudaError_t run_one(const LayerDev& L, const WorkItem& wi, int T, int mode, const himuon_hparams& hp, char* scratch,
@@ -230,11 +366,25 @@ cudaError_t run_one(const LayerDev& L, const WorkItem& wi, int T, int mode, cons
 
 }  // namespace
 
-// Host walk over the work items of one chunk (host copies of the layer table and of the items).
-cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_host, long long n_items, int T, int mode,
-                          int dtype, const himuon_hparams& hp, void* scratch, cudaStream_t s, long long* launches) {
+// One chunk of the work list.  Uniform tiles (T <= 512) run in sub-batches of as many tiles as the scratch holds;
+// whole-matrix items run one at a time (host copies of the layer table and of the items are needed for those).
+cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_host, const LayerDev* layers_dev,
+                          const WorkItem* items_dev, long long n_items, int T, int mode, int dtype,
+                          const himuon_hparams& hp, void* scratch, size_t scratch_bytes, cudaStream_t s, long long* launches) {
   if (n_items < 1) return cudaSuccess;
   if (!cublas().ok) return cudaErrorNotSupported;
+  if (T <= 512 && items_dev) {
+    const size_t per = gemm_path_batch_item_bytes(T);
+    if (scratch_bytes < per + kCublasWs) return cudaErrorInvalidValue;
+    const long long cap = (long long)((scratch_bytes - kCublasWs) / per);
+    for (long long i = 0; i < n_items; i += cap) {
+      const int nb = (int)std::min<long long>(cap, n_items - i);
+      cudaError_t e = dtype == HIMUON_F32 ? run_batch<float>(layers_dev, items_dev + i, nb, T, mode, hp, (char*)scratch, s, launches)
+                                          : run_batch<__nv_bfloat16>(layers_dev, items_dev + i, nb, T, mode, hp, (char*)scratch, s, launches);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+  }
   for (long long i = 0; i < n_items; ++i) {
     const WorkItem& wi = items_host[i];
     const LayerDev& L = layers_host[wi.layer];

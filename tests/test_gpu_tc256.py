@@ -111,9 +111,10 @@ def test_ns_tiles_bf16_256():
         assert e <= PU.TOL_TC, f"tile {i}: {e:.3e}"
 
 
-def test_tc256_unsupported_width_is_refused():
-    """bf16 widths that are not a multiple of 8 have no T = 256 kernel: refused at plan time, never launched."""
+def test_t256_width_not_multiple_of_8_runs_on_the_large_tile_path():
+    """bf16 widths that are not a multiple of 8 have no TMA path at T = 256: served by the large-tile (cuBLAS) path."""
     _need_gpu()
-    G = torch.zeros(300, 300, dtype=torch.bfloat16, device=DEV)
-    with pytest.raises(hm.HimuonError):
-        hm.Plan.from_tensors([torch.empty_like(G)], [G], None, 256)
+    G = _inputs(300, 300, 65)
+    hp = hm.HParams(K=5, eps=1e-7)
+    U = _run_phi(G, 256, hp)
+    PU.check_phi(U, G, 256, hp, PU.TOL_TC, out_is_bf16=True)

@@ -54,10 +54,14 @@ typedef enum { HIMUON_F32 = 0, HIMUON_BF16 = 1 } himuon_dtype;
  *            T = 64       tcgen05, two tiles stacked per 128-lane MMA      (W % 8 == 0, ptr and ld*2 16-byte aligned)
  *            T = 128      tcgen05, operands and accumulator in TMEM        (same)
  *            T = 256      tcgen05 cta_group::2, one tile per CTA pair      (same)
- *          a bf16 matrix whose width is not a multiple of 8 is served by the fp32 kernel at T = 64, 128 and is
- *          HIMUON_ERR_UNSUPPORTED at T = 256;
+ *            T = 512 and the full-matrix branch T >= max(H,W) > 256: large-tile path - fused prep / update
+ *                         kernels around cuBLAS GEMMs (fp32 data, TF32 tensor-core math), tiles staged in
+ *                         sub-batches inside the caller's workspace (himuon_plan_info reports the bytes)
+ *          a bf16 matrix whose width is not a multiple of 8 is served by the fp32 kernel at T = 64, 128 and by
+ *          the large-tile path at T = 256;
  *          fp32 storage -> fp32 path.
- *   FP32 : true fp32 FMA arithmetic for any storage dtype, T in {16, 32, 64, 128} (the <= 1e-4 path). */
+ *   FP32 : true fp32 arithmetic for any storage dtype: FMA kernel for T in {16, 32, 64, 128}, the large-tile
+ *          path with true-fp32 cuBLAS products for T = 256, 512 and the full-matrix branch (the <= 1e-4 path). */
 typedef enum { HIMUON_PATH_AUTO = 0, HIMUON_PATH_FP32 = 1 } himuon_path;
 
 /* {ptr, H, W, ld, dtype}: one row-major device matrix. */
@@ -102,7 +106,8 @@ typedef struct himuon_plan himuon_plan;
  * Supported T: 16, 32, 64, 128 (and 256 where the build provides it; else HIMUON_ERR_UNSUPPORTED).
  * A layer with T >= max(H,W) is the full-matrix branch: it is run as ONE padded
  * tile of the smallest supported size >= max(H,W) with tau = scale_c*sqrt(max(H,W)); if
- * max(H,W) exceeds the largest supported tile the call returns HIMUON_ERR_UNSUPPORTED.
+ * max(H,W) exceeds the largest tile size (512) it is one whole-matrix item of the large-tile path.
+ * Tile sizes: 16, 32, 64, 128, 256, 512 (any T >= max(H,W) selects the full-matrix branch).
  * Tensor-core path needs 16-byte aligned pointers and ld*2 a multiple of 16 (TMA), else
  * HIMUON_ERR_UNSUPPORTED.  Pointers may be NULL when the plan is only inspected (info/worklist);
  * such a plan cannot be bound.  On success *out owns host memory; free with himuon_plan_destroy. */

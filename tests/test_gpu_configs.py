@@ -89,12 +89,12 @@ def test_config4_gpt2_xl_ragged_capped():
     assert plan.workspace_bytes <= 256 << 20
 
 
-@pytest.mark.parametrize("T", [128, 64, 256])
+@pytest.mark.parametrize("T", [128, 64, 256, 32, 16])
 def test_config5_llama3_8b_step(T):
     """BASELINE configs[4] at full size (425 984 tiles at T = 128), 2 GB workspace cap: bench.py's launch."""
     _need_gpu(120)
     plan, worst, n = _run_config_step(I.llama3_8b_spec(), T, 2048, 128, 5)
-    assert plan.n_tiles == {128: 425984, 64: 1703936, 256: 106496}[T]
+    assert plan.n_tiles == {128: 425984, 64: 1703936, 256: 106496, 32: 6815744, 16: 27262976}[T]
     assert plan.workspace_bytes <= 2048 << 20
 
 
@@ -128,3 +128,27 @@ def test_config3_sweep_sampled(T):
         worst = max(worst, e)
     assert worst <= PU.TOL_TC, f"T={T}: worst sampled tile error {worst:.3e}"
     assert bool(torch.isfinite(U.float()).all())
+
+
+@pytest.mark.parametrize("T", [16, 32, 64, 128, 256, 512])
+def test_step_is_deterministic_at_scale(T):
+    """The same step from the same bits twice: bitwise identical W' and M' (no race between the tiles in flight,
+    the prefetches and the stores; fixed summation orders).  GPT-2-XL shapes: ragged at every T >= 128."""
+    _need_gpu(40)
+    spec = I.gpt2_xl_spec(n_blocks=4)
+    hp = hm.HParams(K=5, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
+    outs = []
+    for rep in range(2):
+        Ws, Gs, Ms = [], [], []
+        for i in range(len(spec.layers)):
+            W, G, M = I.make_layer_tensors(spec, i, dtype=torch.bfloat16, device=DEV)
+            Ws.append(W); Gs.append(G); Ms.append(M)
+        plan = hm.Plan.from_tensors(Ws, Gs, Ms, T, workspace_cap_bytes=1024 << 20).bind()
+        plan.step(hp)
+        plan.step(hp)                      # second step on the updated state
+        torch.cuda.synchronize()
+        outs.append((Ws, Ms))
+        plan.destroy()
+    for a, b in zip(outs[0][0] + outs[0][1], outs[1][0] + outs[1][1]):
+        assert torch.equal(a, b)
+        assert bool(torch.isfinite(a.float()).all())

@@ -401,7 +401,7 @@ def main():
     ap.add_argument("--T", type=int, default=128)
     ap.add_argument("--K", type=int, default=5)
     ap.add_argument("--cap-mb", type=int, default=2048)
-    ap.add_argument("--cpu-tiles", type=int, default=4096)
+    ap.add_argument("--cpu-tiles", type=int, default=16384)
     ap.add_argument("--e2e-host-gb", type=float, default=8.0)
     ap.add_argument("--blocks", type=int, default=0, help="truncate the parameter set to its first N transformer blocks (profiling only)")
     ap.add_argument("--shard", action="store_true", help="N > 1: split the parameter set over the ranks by whole matrices (strong scaling)")

@@ -180,6 +180,47 @@ def step(W: np.ndarray, G: np.ndarray, M_prev: np.ndarray, hp: HParams, T: Optio
     return W_new, M, U
 
 
+# ----------------------------------------------------------------------------- rectangular tiles (T_h, T_w)
+
+def phi_tiled_rect(A: np.ndarray, Th: int, Tw: int, K: int = 5, a: float = NS_A, b: float = NS_B,
+                   c: float = NS_C, eps: float = 0.0) -> np.ndarray:
+    """Tiled map with rectangular tiles (T_h, T_w) ("Rectangular tiles (T_h, T_w) are used only in the
+    tile-shape study of Figure 8; elsewhere T_h = T_w = T").
+
+    The same construction as B_T with the two tile extents decoupled: zero-pad to (R T_h) x (C T_w),
+    R = ceil(H / T_h), C = ceil(W / T_w), apply Phi_K to every T_h x T_w tile (Phi_K transposes a tall tile
+    internally), reassemble, remove the padding.  T_h >= H and T_w >= W is one tile = the whole
+    matrix, i.e. the full-matrix branch."""
+    A = np.asarray(A, dtype=np.float64)
+    H, W = A.shape
+    R, C = -(-H // Th), -(-W // Tw)
+    P = np.zeros((R * Th, C * Tw), dtype=np.float64)
+    P[:H, :W] = A
+    Q = np.empty_like(P)
+    for r in range(R):
+        for cc in range(C):
+            Q[r * Th:(r + 1) * Th, cc * Tw:(cc + 1) * Tw] = phi(P[r * Th:(r + 1) * Th, cc * Tw:(cc + 1) * Tw], K, a, b, c, eps)
+    return Q[:H, :W].copy()
+
+
+def tau_rect(H: int, W: int, Th: int, Tw: int, scale_c: float = 0.2) -> float:
+    """tau = c sqrt(max(T_h, T_w)) for rectangular tiles; c sqrt(max(H, W)) when one tile covers
+    the matrix (full-matrix branch)."""
+    if Th >= H and Tw >= W:
+        return scale_c * math.sqrt(max(H, W))
+    return scale_c * math.sqrt(max(Th, Tw))
+
+
+def step_rect(W: np.ndarray, G: np.ndarray, M_prev: np.ndarray, hp: "HParams", Th: int, Tw: int):
+    """Algorithm 4.1 with rectangular tiles: momentum, Phi over (T_h, T_w) tiles, update
+    W' = (1 - lr wd) W - lr tau U (Eq. 4.6) with tau_rect.  Returns (W', M', U)."""
+    M_new, G_hat = momentum(G, M_prev, hp.beta, hp.nesterov)
+    U = phi_tiled_rect(G_hat, Th, Tw, hp.K, hp.a, hp.b, hp.c, hp.eps)
+    t = tau_rect(G.shape[0], G.shape[1], Th, Tw, hp.scale_c)
+    W_new = (1.0 - hp.lr * hp.wd) * np.asarray(W, dtype=np.float64) - hp.lr * t * U
+    return W_new, M_new, U
+
+
 # ----------------------------------------------------------------------------- execution plan (host logic)
 
 def enumerate_tiles(shapes: Sequence[Tuple[int, int]], T_per_layer: Sequence[Optional[int]]) -> List[Tuple[int, int, int]]:

@@ -347,3 +347,55 @@ def test_per_tile_error_metric():
     e = O.per_tile_rel_fro_error(Bm, A, 4)
     assert e.shape == (2, 2)
     assert e[0, 1] == pytest.approx(0.1) and e[0, 0] == 0 and e[1, 1] == 0
+
+
+# ----------------------------------------------------------------------------- rectangular tiles
+
+def test_rect_tiles_reduce_to_square_and_to_full():
+    rng = np.random.default_rng(31)
+    A = rng.standard_normal((50, 70))
+    for T in (16, 32):
+        assert np.array_equal(O.phi_tiled_rect(A, T, T), O.phi_tiled(A, T))          # T_h = T_w = T
+    assert np.max(np.abs(O.phi_tiled_rect(A, 64, 128) - O.phi(A))) < 1e-12            # one (padded) tile covers the matrix
+    assert O.tau_rect(50, 70, 64, 128) == pytest.approx(0.2 * math.sqrt(70))          # full branch
+    assert O.tau_rect(500, 700, 16, 64) == pytest.approx(0.2 * 8.0)                   # c sqrt(max(T_h, T_w))
+    assert O.tau_rect(500, 700, 64, 16) == pytest.approx(0.2 * 8.0)
+
+
+def test_rect_tiles_blockwise_definition_and_independence():
+    """Every T_h x T_w block of the output is Phi_K of the same block of the (padded) input, computed from
+    scratch here with numpy slicing and the SVD closed form; perturbing one block changes only that block."""
+    rng = np.random.default_rng(32)
+    H, W, Th, Tw = 40, 90, 16, 32
+    A = rng.standard_normal((H, W))
+    U = O.phi_tiled_rect(A, Th, Tw)
+    for r in range(-(-H // Th)):
+        for c in range(-(-W // Tw)):
+            blk = A[r * Th:(r + 1) * Th, c * Tw:(c + 1) * Tw]                         # ragged at the edges: unpadded block
+            u, s, vt = np.linalg.svd(blk, full_matrices=False)
+            x = s / np.linalg.norm(s)
+            for _ in range(5):
+                x = O.NS_A * x + O.NS_B * x ** 3 + O.NS_C * x ** 5
+            want = (u * x) @ vt
+            got = U[r * Th:(r + 1) * Th, c * Tw:(c + 1) * Tw]
+            assert np.max(np.abs(got - want)) < 1e-10
+    B = A.copy()
+    B[16:32, 32:64] += rng.standard_normal((16, 32))
+    V = O.phi_tiled_rect(B, Th, Tw)
+    mask = np.ones((H, W), dtype=bool)
+    mask[16:32, 32:64] = False
+    assert np.array_equal(U[mask], V[mask]) and not np.array_equal(U[~mask], V[~mask])
+
+
+def test_rect_tiles_transpose_equivariance_and_step():
+    rng = np.random.default_rng(33)
+    A = rng.standard_normal((48, 80))
+    assert np.max(np.abs(O.phi_tiled_rect(A.T, 32, 16) - O.phi_tiled_rect(A, 16, 32).T)) < 1e-12
+    hp = O.HParams(lr=0.02, beta=0.95, nesterov=True, wd=0.01, K=5)
+    W0, G, M0 = rng.standard_normal((48, 80)), rng.standard_normal((48, 80)), rng.standard_normal((48, 80))
+    W1, M1, U = O.step_rect(W0, G, M0, hp, 16, 32)
+    assert np.array_equal(M1, 0.95 * M0 + G)
+    assert np.max(np.abs(W1 - ((1 - 0.02 * 0.01) * W0 - 0.02 * 0.2 * math.sqrt(32) * U))) < 1e-14
+    Ws, Ms, Us = O.step(W0, G, M0, hp, 16)
+    Wr, Mr, Ur = O.step_rect(W0, G, M0, hp, 16, 16)
+    assert np.array_equal(Ws, Wr) and np.array_equal(Us, Ur)

@@ -74,10 +74,15 @@ typedef struct {
 
 /* One 2-D parameter l of Algorithm 4.1: weight W_l, gradient G_l, momentum M_l (same H, W, dtype).
  * T = 0 selects the plan-wide default; otherwise this layer's tile size (runtime tile schedule).
+ * T_w = 0 (or T_w == T): square T x T tiles.  Otherwise rectangular tiles of T rows x T_w columns (PAPER.md:55,
+ * the tile-shape study of Fig. 8): both extents powers of two in 16..2048, R = ceil(H/T), C = ceil(W/T_w),
+ * tau = scale_c*sqrt(max(T, T_w)); served by the large-tile path (cuBLAS products, Gram matrix on
+ * the short side of the tile).
  * For himuon_phi only g (input) and w (output) are used; m may be {NULL,...}. */
 typedef struct {
   himuon_mat w, g, m;
   int32_t    T;
+  int32_t    T_w;
 } himuon_layer;
 
 /* Hyper-parameters of Algorithm 4.1 (defaults).

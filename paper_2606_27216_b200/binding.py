@@ -37,7 +37,7 @@ class himuon_mat(C.Structure):
 
 
 class himuon_layer(C.Structure):
-    _fields_ = [("w", himuon_mat), ("g", himuon_mat), ("m", himuon_mat), ("T", C.c_int32)]
+    _fields_ = [("w", himuon_mat), ("g", himuon_mat), ("m", himuon_mat), ("T", C.c_int32), ("T_w", C.c_int32)]
 
 
 class himuon_hparams(C.Structure):
@@ -205,11 +205,14 @@ class Plan:
 
     @classmethod
     def from_tensors(cls, Ws, Gs, Ms, T_default: int, T_per_layer: Optional[Sequence[int]] = None,
-                     path: int = HIMUON_PATH_AUTO, workspace_cap_bytes: int = 0) -> "Plan":
+                     path: int = HIMUON_PATH_AUTO, workspace_cap_bytes: int = 0,
+                     Tw_per_layer: Optional[Sequence[int]] = None) -> "Plan":
+        """Tw_per_layer: tile width per layer for rectangular tiles (T rows x T_w columns); 0 / None = square."""
         layers = []
         for i, (w, g) in enumerate(zip(Ws, Gs)):
             m = Ms[i] if Ms is not None else None
-            layers.append(himuon_layer(mat_of(w), mat_of(g), mat_of(m), T_per_layer[i] if T_per_layer else 0))
+            layers.append(himuon_layer(mat_of(w), mat_of(g), mat_of(m), T_per_layer[i] if T_per_layer else 0,
+                                       Tw_per_layer[i] if Tw_per_layer else 0))
         p = cls(layers, T_default, path, workspace_cap_bytes)
         p._keep = [Ws, Gs, Ms]
         return p

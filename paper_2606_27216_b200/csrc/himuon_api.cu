@@ -189,6 +189,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
   p->cap = workspace_cap_bytes;
   p->layers.assign(layers, layers + n_layers);
   p->T_eff.resize(n_layers);
+  p->Tw_eff.resize(n_layers);
   p->kpath.resize(n_layers);
   p->layer_dev.resize(n_layers);
 
@@ -202,11 +203,17 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
     if (L.m.ptr && (L.m.H != H || L.m.W != W || L.m.dtype != dt)) { st = HIMUON_ERR_INVALID_ARG; break; }
     if (L.g.ld < W || L.w.ld < W || (L.m.ptr && L.m.ld < W)) { st = HIMUON_ERR_INVALID_ARG; break; }
     int T = L.T > 0 ? L.T : T_default;
-    if (T <= 0 || L.T < 0) { st = HIMUON_ERR_INVALID_ARG; break; }
+    if (T <= 0 || L.T < 0 || L.T_w < 0) { st = HIMUON_ERR_INVALID_ARG; break; }
     const int  mx = H > W ? H : W;
-    const bool full = T >= mx;   // full-matrix branch
-    int Te;
-    if (full) {
+    const bool rect = L.T_w > 0 && L.T_w != T && !(T >= H && L.T_w >= W);   // rectangular tiles
+    const bool full = rect ? false : (L.T_w > 0 && L.T_w != T ? true : T >= mx);   // full-matrix branch
+    int Te, Twe = 0;
+    if (rect) {
+      auto pow2_ok = [](int v) { return v >= 16 && v <= 2048 && (v & (v - 1)) == 0; };
+      if (!pow2_ok(T) || !pow2_ok(L.T_w)) { st = HIMUON_ERR_INVALID_ARG; break; }
+      Te = T;
+      Twe = L.T_w;
+    } else if (full) {
       Te = smallest_supported_T_at_least(mx, dt, path);
       if (Te < 0) Te = kWholeMatrixT;          // larger than every tile size: one whole-matrix item on the cuBLAS path
     } else {
@@ -216,17 +223,19 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       if (select_kpath(dt, path, T) < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
       Te = T;
     }
-    const int kp = select_kpath(dt, path, Te, W);
+    const int kp = rect ? KPATH_GEMM : select_kpath(dt, path, Te, W);
     if (kp < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
+    if (!rect) Twe = Te;
     if (kp == KPATH_GEMM) {
       size_t need;
-      if (Te <= 512) {   // uniform tiles run in sub-batches: as many tiles as a scratch budget holds (>= 1)
-        const size_t per = gemm_path_batch_item_bytes(Te);
+      if (Te <= 2048 && Twe <= 2048) {   // uniform tiles run in sub-batches: as many tiles as a scratch budget holds (>= 1)
+        const size_t per = gemm_path_batch_item_bytes(Te, Twe);
         size_t       budget = (size_t)512 << 20;
         if (workspace_cap_bytes && workspace_cap_bytes / 2 < budget) budget = workspace_cap_bytes / 2;
-        gemm_tiles[Te] += (long long)((H + Te - 1) / Te) * ((W + Te - 1) / Te);
+        const int key = Te * 4096 + Twe;
+        gemm_tiles[key] += (long long)((H + Te - 1) / Te) * ((W + Twe - 1) / Twe);
         long long nb = (long long)(budget / per);
-        if (nb > gemm_tiles[Te]) nb = gemm_tiles[Te];
+        if (nb > gemm_tiles[key]) nb = gemm_tiles[key];
         if (nb < 1) nb = 1;
         need = gemm_path_fixed_bytes() + (size_t)nb * per;
       } else {
@@ -235,6 +244,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       if (need > p->scratch_bytes) p->scratch_bytes = need;
     }
     p->T_eff[l] = Te;
+    p->Tw_eff[l] = Twe;
     p->kpath[l] = kp;
     if (!L.g.ptr || !L.w.ptr) p->bindable = false;
     const size_t esz = dt == HIMUON_BF16 ? 2 : 4;
@@ -254,7 +264,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
     D.w = L.w.ptr; D.g = L.g.ptr; D.m = L.m.ptr;
     D.ld_w = L.w.ld; D.ld_g = L.g.ld; D.ld_m = L.m.ptr ? L.m.ld : 0;
     D.H = H; D.W = W; D.dtype = dt;
-    D.tau_base = std::sqrt((float)(full ? mx : T));
+    D.tau_base = std::sqrt((float)(full ? mx : (rect ? (T > L.T_w ? T : L.T_w) : T)));
   }
   if (st != HIMUON_OK) { delete p; return st; }
 
@@ -262,15 +272,17 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
   for (int l = 0; l < n_layers; ++l) {
     int dt = layers[l].g.dtype, bi = -1;
     for (size_t b = 0; b < p->buckets.size(); ++b)
-      if (p->buckets[b].T == p->T_eff[l] && p->buckets[b].dtype == dt && p->buckets[b].kpath == p->kpath[l]) bi = (int)b;
-    if (bi < 0) p->buckets.push_back(Bucket{p->T_eff[l], dt, p->kpath[l], 0, 0});
+      if (p->buckets[b].T == p->T_eff[l] && p->buckets[b].Tw == p->Tw_eff[l] && p->buckets[b].dtype == dt &&
+          p->buckets[b].kpath == p->kpath[l])
+        bi = (int)b;
+    if (bi < 0) p->buckets.push_back(Bucket{p->T_eff[l], p->Tw_eff[l], dt, p->kpath[l], 0, 0});
   }
   for (size_t b = 0; b < p->buckets.size(); ++b) {
     Bucket& B = p->buckets[b];
     B.begin = (long long)p->items.size();
     for (int l = 0; l < n_layers; ++l) {
-      if (p->T_eff[l] != B.T || layers[l].g.dtype != B.dtype || p->kpath[l] != B.kpath) continue;
-      const int R = (layers[l].g.H + B.T - 1) / B.T, C = (layers[l].g.W + B.T - 1) / B.T;
+      if (p->T_eff[l] != B.T || p->Tw_eff[l] != B.Tw || layers[l].g.dtype != B.dtype || p->kpath[l] != B.kpath) continue;
+      const int R = (layers[l].g.H + B.T - 1) / B.T, C = (layers[l].g.W + B.Tw - 1) / B.Tw;
       for (int r = 0; r < R; ++r)
         for (int c = 0; c < C; ++c) p->items.push_back(WorkItem{l, r, c, 0});
     }
@@ -412,7 +424,7 @@ static himuon_status run_plan(himuon_plan* plan, const himuon_hparams* hp, int m
     if (B.kpath == KPATH_GEMM) {   // large tiles: products go to cuBLAS (sub-batches of tiles / whole matrices)
       long long   n_launch = 0;
       cudaError_t e = run_gemm_path(plan->layer_dev.data(), plan->items.data() + c.begin, a.layers, a.items,
-                                    c.end - c.begin, B.T, mode, B.dtype, *hp, ws + plan->off_scratch,
+                                    c.end - c.begin, B.T, B.Tw, mode, B.dtype, *hp, ws + plan->off_scratch,
                                     plan->scratch_bytes, s, &n_launch);
       g_launches.fetch_add(n_launch);
       if (e != cudaSuccess) return cuda_fail(e, "step: large-tile path (cuBLAS)");
@@ -479,7 +491,7 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
     cudaError_t eg = cudaMemcpyAsync(ws, &D, sizeof(D), cudaMemcpyHostToDevice, s);
     if (eg != cudaSuccess) return cuda_fail(eg, "ns_tiles: layer table");
     // one tile per sub-batch: an implicit work list is not available on the device, so each tile is one whole block
-    eg = run_gemm_path(&D, its.data(), (const LayerDev*)ws, nullptr, n_tiles, T, MODE_PHI, dtype, hp,
+    eg = run_gemm_path(&D, its.data(), (const LayerDev*)ws, nullptr, n_tiles, T, T, MODE_PHI, dtype, hp,
                        ws + align_up(128 + 3 * sizeof(CUtensorMap), 256), gemm_path_scratch_bytes(512, 512), s, &n_launch);
     g_launches.fetch_add(n_launch);
     if (eg != cudaSuccess) return cuda_fail(eg, "ns_tiles: large-tile path (cuBLAS)");

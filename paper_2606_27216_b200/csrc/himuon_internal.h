@@ -61,10 +61,10 @@ cudaError_t launch_warp(const LaunchArgs& a, cudaStream_t stream);
 
 // kernels_gemm.cu -- large tiles (T = 512, full-matrix branch beyond 256): cuBLAS products, host walk over the items.
 size_t      gemm_path_scratch_bytes(int h, int w);        // one whole h x w block at a time
-size_t      gemm_path_batch_item_bytes(int T);            // per tile of a sub-batch of uniform tiles (T <= 512)
+size_t      gemm_path_batch_item_bytes(int Th, int Tw);   // per tile of a sub-batch of uniform Th x Tw tiles
 size_t      gemm_path_fixed_bytes();                      // cuBLAS workspace inside the scratch
 cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_host, const LayerDev* layers_dev,
-                          const WorkItem* items_dev, long long n_items, int T, int mode, int dtype,
+                          const WorkItem* items_dev, long long n_items, int T, int Tw, int mode, int dtype,
                           const himuon_hparams& hp, void* scratch, size_t scratch_bytes, cudaStream_t stream,
                           long long* launches);
 
@@ -74,7 +74,8 @@ void note_launch();
 // ---- host plan --------------------------------------------------------------------------------
 
 struct Bucket {
-  int       T;
+  int       T;            // tile rows
+  int       Tw;           // tile columns (= T except for rectangular tiles)
   int       dtype;
   int       kpath;
   long long begin, end;   // range in the work list
@@ -89,7 +90,8 @@ struct Chunk {
 
 struct himuon_plan {
   std::vector<himuon_layer>     layers;
-  std::vector<int>              T_eff;       // per layer, effective (supported) tile size
+  std::vector<int>              T_eff;       // per layer, effective (supported) tile size (rows)
+  std::vector<int>              Tw_eff;      // per layer, tile columns (= T_eff except for rectangular tiles)
   std::vector<int>              kpath;       // per layer
   std::vector<himuon::LayerDev> layer_dev;
   std::vector<himuon::WorkItem> items;       // execution order

@@ -160,16 +160,16 @@ constexpr int kTileBlocks = 32;
 template <typename S>
 __global__ void __launch_bounds__(kEwThreads)
 k_prep_b(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, float* __restrict__ X,
-         float* __restrict__ partial, int T, int step_mode, float beta, int nesterov) {
+         float* __restrict__ partial, int Th, int Tw, long long stride, int step_mode, float beta, int nesterov) {
   const WorkItem wi = items[blockIdx.y];
   const LayerDev L = layers[wi.layer];
-  const int row0 = wi.r * T, col0 = wi.c * T;
+  const int row0 = wi.r * Th, col0 = wi.c * Tw;
   const S* G = reinterpret_cast<const S*>(L.g);
   S* M = reinterpret_cast<S*>(L.m);
-  float* Xt = X + (long long)blockIdx.y * T * T;
+  float* Xt = X + (long long)blockIdx.y * stride;
   float ss = 0.f;
-  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < T * T; i += kTileBlocks * kEwThreads) {
-    const int r = i / T, c = i - r * T;
+  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < Th * Tw; i += kTileBlocks * kEwThreads) {
+    const int r = i / Tw, c = i - r * Tw;
     float x = 0.f;
     if (row0 + r < L.H && col0 + c < L.W) {
       const float g = ld_elem(G + (long long)(row0 + r) * L.ld_g + col0 + c);
@@ -198,33 +198,33 @@ k_prep_b(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items
 }
 
 __global__ void __launch_bounds__(kEwThreads)
-k_scale_b(float* __restrict__ X, const float* __restrict__ partial, int T, float eps) {
+k_scale_b(float* __restrict__ X, const float* __restrict__ partial, int n, long long stride, float eps) {
   float tot = 0.f;
 #pragma unroll
   for (int i = 0; i < kTileBlocks; ++i) tot += partial[blockIdx.y * kTileBlocks + i];   // same order in every thread
   const float nrm = sqrtf(tot);
   const float inv = nrm > 0.f ? 1.f / (nrm + eps) : 0.f;
-  float* Xt = X + (long long)blockIdx.y * T * T;
-  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < T * T; i += kTileBlocks * kEwThreads) Xt[i] *= inv;
+  float* Xt = X + (long long)blockIdx.y * stride;
+  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < n; i += kTileBlocks * kEwThreads) Xt[i] *= inv;
 }
 
-__global__ void k_add_diag_b(float* __restrict__ B, int T, float a) {
+__global__ void k_add_diag_b(float* __restrict__ B, int T, long long stride, float a) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < T) B[(long long)blockIdx.y * T * T + (long long)i * T + i] += a;
+  if (i < T) B[(long long)blockIdx.y * stride + (long long)i * T + i] += a;
 }
 
 template <typename S>
 __global__ void __launch_bounds__(kEwThreads)
-k_update_b(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, const float* __restrict__ X, int T,
-           int step_mode, float keep, float lr_scale) {
+k_update_b(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, const float* __restrict__ X, int Th,
+           int Tw, long long stride, int step_mode, float keep, float lr_scale) {
   const WorkItem wi = items[blockIdx.y];
   const LayerDev L = layers[wi.layer];
-  const int row0 = wi.r * T, col0 = wi.c * T;
+  const int row0 = wi.r * Th, col0 = wi.c * Tw;
   S* W = reinterpret_cast<S*>(L.w);
-  const float* Xt = X + (long long)blockIdx.y * T * T;
+  const float* Xt = X + (long long)blockIdx.y * stride;
   const float stepsz = lr_scale * L.tau_base;
-  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < T * T; i += kTileBlocks * kEwThreads) {
-    const int r = i / T, c = i - r * T;
+  for (int i = blockIdx.x * kEwThreads + threadIdx.x; i < Th * Tw; i += kTileBlocks * kEwThreads) {
+    const int r = i / Tw, c = i - r * Tw;
     if (row0 + r < L.H && col0 + c < L.W) {
       S* p = W + (long long)(row0 + r) * L.ld_w + col0 + c;
       st_elem(p, step_mode ? fmaf(keep, ld_elem(p), stepsz * Xt[i]) : Xt[i]);
@@ -245,27 +245,33 @@ size_t gemm_path_scratch_bytes(int h, int w) {
 
 // Scratch bytes per tile of the batched form: X, X2, A, B (T x T fp32 each) and the partial sums.
 size_t gemm_path_fixed_bytes() { return kCublasWs; }
-size_t gemm_path_batch_item_bytes(int T) { return 4 * align256((size_t)T * T * 4) + align256(kTileBlocks * 4); }
+size_t gemm_path_batch_item_bytes(int Th, int Tw) {
+  const size_t r = (size_t)std::min(Th, Tw);
+  return 2 * align256((size_t)Th * Tw * 4) + 2 * align256(r * r * 4) + align256(kTileBlocks * 4);
+}
 
 namespace {
 
-// One sub-batch of nb uniform T x T tiles (items_dev / layers_dev: device copies of the work items and layer table).
+// One sub-batch of nb uniform Th x Tw tiles, staged zero-padded (items_dev / layers_dev: device copies of the work
+// items and of the layer table).  Gram matrix on the short side of the tile.
 template <typename S>
-cudaError_t run_batch(const LayerDev* layers_dev, const WorkItem* items_dev, int nb, int T, int mode,
+cudaError_t run_batch(const LayerDev* layers_dev, const WorkItem* items_dev, int nb, int Th, int Tw, int mode,
                       const himuon_hparams& hp, char* scratch, cudaStream_t s, long long* launches) {
   Cublas& cb = cublas();
-  const size_t tb = align256((size_t)T * T * 4);
+  const int r = std::min(Th, Tw);
+  const size_t xb = align256((size_t)Th * Tw * 4), ab = align256((size_t)r * r * 4);
   float* X = reinterpret_cast<float*>(scratch);
-  float* X2 = reinterpret_cast<float*>(scratch + (size_t)nb * tb);
-  float* A = reinterpret_cast<float*>(scratch + 2 * (size_t)nb * tb);
-  float* B = reinterpret_cast<float*>(scratch + 3 * (size_t)nb * tb);
-  float* partial = reinterpret_cast<float*>(scratch + 4 * (size_t)nb * tb);
-  void* cws = scratch + 4 * (size_t)nb * tb + (size_t)nb * align256(kTileBlocks * 4);
+  float* X2 = reinterpret_cast<float*>(scratch + (size_t)nb * xb);
+  float* A = reinterpret_cast<float*>(scratch + 2 * (size_t)nb * xb);
+  float* B = reinterpret_cast<float*>(scratch + 2 * (size_t)nb * xb + (size_t)nb * ab);
+  float* partial = reinterpret_cast<float*>(scratch + 2 * (size_t)nb * (xb + ab));
+  void* cws = scratch + 2 * (size_t)nb * (xb + ab) + (size_t)nb * align256(kTileBlocks * 4);
   const bool step_mode = (mode == MODE_STEP);
-  const long long stride = (long long)(tb / 4);
+  const long long sx = (long long)(xb / 4), sa = (long long)(ab / 4);
+  const int h = Th, w = Tw;
   const dim3 grid(kTileBlocks, nb);
-  k_prep_b<S><<<grid, kEwThreads, 0, s>>>(layers_dev, items_dev, X, partial, T, step_mode ? 1 : 0, hp.beta, hp.nesterov);
-  k_scale_b<<<grid, kEwThreads, 0, s>>>(X, partial, T, hp.eps);
+  k_prep_b<S><<<grid, kEwThreads, 0, s>>>(layers_dev, items_dev, X, partial, Th, Tw, sx, step_mode ? 1 : 0, hp.beta, hp.nesterov);
+  k_scale_b<<<grid, kEwThreads, 0, s>>>(X, partial, Th * Tw, sx, hp.eps);
   *launches += 2;
   if (hp.K > 0) {
     if (cb.set_stream(cb.handle, s) != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
@@ -273,24 +279,33 @@ cudaError_t run_batch(const LayerDev* layers_dev, const WorkItem* items_dev, int
   }
   const cublasComputeType_t ct = sizeof(S) == 4 ? CUBLAS_COMPUTE_32F : CUBLAS_COMPUTE_32F_FAST_TF32;
   const float one = 1.f, zero = 0.f;
+  // Row-major X (h x w, ld = w) is the column-major w x h matrix Xc = X^T with leading dimension w (see run_one).
   for (int k = 0; k < hp.K; ++k) {
-    // square tiles: A = X X^T = Xc^T Xc; B = b A + c A A + a I; X <- B X, i.e. Xc_new = Xc B (column-major views)
-    cublasStatus_t st = cb.gemm_batched(cb.handle, CUBLAS_OP_T, CUBLAS_OP_N, T, T, T, &one, X, CUDA_R_32F, T, stride, X,
-                                        CUDA_R_32F, T, stride, &zero, A, CUDA_R_32F, T, stride, nb, ct, CUBLAS_GEMM_DEFAULT);
+    cublasStatus_t st;
+    if (h <= w)
+      st = cb.gemm_batched(cb.handle, CUBLAS_OP_T, CUBLAS_OP_N, h, h, w, &one, X, CUDA_R_32F, w, sx, X, CUDA_R_32F, w, sx,
+                           &zero, A, CUDA_R_32F, r, sa, nb, ct, CUBLAS_GEMM_DEFAULT);
+    else
+      st = cb.gemm_batched(cb.handle, CUBLAS_OP_N, CUBLAS_OP_T, w, w, h, &one, X, CUDA_R_32F, w, sx, X, CUDA_R_32F, w, sx,
+                           &zero, A, CUDA_R_32F, r, sa, nb, ct, CUBLAS_GEMM_DEFAULT);
     if (st != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
-    cudaError_t e = cudaMemcpyAsync(B, A, (size_t)nb * tb, cudaMemcpyDeviceToDevice, s);
+    cudaError_t e = cudaMemcpyAsync(B, A, (size_t)nb * ab, cudaMemcpyDeviceToDevice, s);
     if (e != cudaSuccess) return e;
-    st = cb.gemm_batched(cb.handle, CUBLAS_OP_N, CUBLAS_OP_N, T, T, T, &hp.c, A, CUDA_R_32F, T, stride, A, CUDA_R_32F, T,
-                         stride, &hp.b, B, CUDA_R_32F, T, stride, nb, ct, CUBLAS_GEMM_DEFAULT);
+    st = cb.gemm_batched(cb.handle, CUBLAS_OP_N, CUBLAS_OP_N, r, r, r, &hp.c, A, CUDA_R_32F, r, sa, A, CUDA_R_32F, r, sa,
+                         &hp.b, B, CUDA_R_32F, r, sa, nb, ct, CUBLAS_GEMM_DEFAULT);
     if (st != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
-    k_add_diag_b<<<dim3((T + 255) / 256, nb), 256, 0, s>>>(B, T, hp.a);
-    st = cb.gemm_batched(cb.handle, CUBLAS_OP_N, CUBLAS_OP_N, T, T, T, &one, X, CUDA_R_32F, T, stride, B, CUDA_R_32F, T,
-                         stride, &zero, X2, CUDA_R_32F, T, stride, nb, ct, CUBLAS_GEMM_DEFAULT);
+    k_add_diag_b<<<dim3((r + 255) / 256, nb), 256, 0, s>>>(B, r, sa, hp.a);
+    if (h <= w)
+      st = cb.gemm_batched(cb.handle, CUBLAS_OP_N, CUBLAS_OP_N, w, h, h, &one, X, CUDA_R_32F, w, sx, B, CUDA_R_32F, r, sa,
+                           &zero, X2, CUDA_R_32F, w, sx, nb, ct, CUBLAS_GEMM_DEFAULT);
+    else
+      st = cb.gemm_batched(cb.handle, CUBLAS_OP_N, CUBLAS_OP_N, w, h, w, &one, B, CUDA_R_32F, r, sa, X, CUDA_R_32F, w, sx,
+                           &zero, X2, CUDA_R_32F, w, sx, nb, ct, CUBLAS_GEMM_DEFAULT);
     if (st != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
     std::swap(X, X2);
     *launches += 5;
   }
-  k_update_b<S><<<grid, kEwThreads, 0, s>>>(layers_dev, items_dev, X, T, step_mode ? 1 : 0, 1.f - hp.lr * hp.wd,
+  k_update_b<S><<<grid, kEwThreads, 0, s>>>(layers_dev, items_dev, X, Th, Tw, sx, step_mode ? 1 : 0, 1.f - hp.lr * hp.wd,
                                             -hp.lr * hp.scale_c);
   *launches += 1;
   return cudaGetLastError();
@@ -369,18 +384,18 @@ cudaError_t run_one(const LayerDev& L, const WorkItem& wi, int T, int mode, cons
 // One chunk of the work list.  Uniform tiles (T <= 512) run in sub-batches of as many tiles as the scratch holds;
 // whole-matrix items run one at a time (host copies of the layer table and of the items are needed for those).
 cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_host, const LayerDev* layers_dev,
-                          const WorkItem* items_dev, long long n_items, int T, int mode, int dtype,
+                          const WorkItem* items_dev, long long n_items, int T, int Tw, int mode, int dtype,
                           const himuon_hparams& hp, void* scratch, size_t scratch_bytes, cudaStream_t s, long long* launches) {
   if (n_items < 1) return cudaSuccess;
   if (!cublas().ok) return cudaErrorNotSupported;
-  if (T <= 512 && items_dev) {
-    const size_t per = gemm_path_batch_item_bytes(T);
+  if (T <= 2048 && Tw <= 2048 && items_dev) {
+    const size_t per = gemm_path_batch_item_bytes(T, Tw);
     if (scratch_bytes < per + kCublasWs) return cudaErrorInvalidValue;
     const long long cap = (long long)((scratch_bytes - kCublasWs) / per);
     for (long long i = 0; i < n_items; i += cap) {
       const int nb = (int)std::min<long long>(cap, n_items - i);
-      cudaError_t e = dtype == HIMUON_F32 ? run_batch<float>(layers_dev, items_dev + i, nb, T, mode, hp, (char*)scratch, s, launches)
-                                          : run_batch<__nv_bfloat16>(layers_dev, items_dev + i, nb, T, mode, hp, (char*)scratch, s, launches);
+      cudaError_t e = dtype == HIMUON_F32 ? run_batch<float>(layers_dev, items_dev + i, nb, T, Tw, mode, hp, (char*)scratch, s, launches)
+                                          : run_batch<__nv_bfloat16>(layers_dev, items_dev + i, nb, T, Tw, mode, hp, (char*)scratch, s, launches);
       if (e != cudaSuccess) return e;
     }
     return cudaSuccess;

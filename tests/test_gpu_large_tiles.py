@@ -80,3 +80,54 @@ def test_ns_tiles_512():
         ref = PU.O.phi(PU.f64(tiles[i]), ohp.K, ohp.a, ohp.b, ohp.c, ohp.eps)
         e = np.linalg.norm(PU.f64(out[i]) - ref) / np.linalg.norm(ref)
         assert e <= PU.TOL_TC, f"tile {i}: {e:.3e}"
+
+
+def _rect_err(U, ref, Th, Tw):
+    H, W = ref.shape
+    worst = 0.0
+    for r in range(-(-H // Th)):
+        for c in range(-(-W // Tw)):
+            a, b = U[r * Th:(r + 1) * Th, c * Tw:(c + 1) * Tw], ref[r * Th:(r + 1) * Th, c * Tw:(c + 1) * Tw]
+            worst = max(worst, np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-30))
+    return worst
+
+
+@pytest.mark.parametrize("H,W,Th,Tw", [(256, 512, 64, 256), (300, 500, 128, 32), (1024, 256, 16, 256), (200, 200, 256, 64)])
+def test_rectangular_tiles_phi(H, W, Th, Tw):
+    """Rectangular tiles (T_h, T_w) of the tile-shape study against phi_tiled_rect."""
+    _need_gpu()
+    G = I.lowrank_plus_noise(H, W, 32, seed_cfg=75, layer_index=0, tensor_id=I.TENSOR_G)
+    Gd = G.to(DEV)
+    Ud = torch.full_like(Gd, float("nan"))
+    hp = hm.HParams(K=5, eps=1e-7)
+    plan = hm.Plan.from_tensors([Ud], [Gd], None, Th, Tw_per_layer=[Tw]).bind()
+    assert plan.n_tiles == -(-H // Th) * -(-W // Tw)
+    plan.phi(hp)
+    torch.cuda.synchronize()
+    ohp = PU.oracle_hp(hp)
+    ref = PU.O.phi_tiled_rect(PU.f64(G), Th, Tw, ohp.K, ohp.a, ohp.b, ohp.c, ohp.eps)
+    assert _rect_err(PU.f64(Ud.cpu()), ref, Th, Tw) <= PU.TOL_TC
+
+
+def test_rectangular_tiles_step():
+    """Full step with rectangular tiles: tau = c sqrt(max(T_h, T_w))."""
+    _need_gpu()
+    H, W, Th, Tw = 384, 320, 128, 64
+    G = I.lowrank_plus_noise(H, W, 32, seed_cfg=76, layer_index=0, tensor_id=I.TENSOR_G)
+    M = I.lowrank_plus_noise(H, W, 32, seed_cfg=76, layer_index=0, tensor_id=I.TENSOR_M)
+    W0 = I.gaussian(H, W, seed_cfg=76, layer_index=0, tensor_id=I.TENSOR_W, dtype=torch.bfloat16, scale=0.02)
+    hp = hm.HParams(K=5, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
+    Wd, Gd, Md = W0.to(DEV), G.to(DEV), M.to(DEV)
+    plan = hm.Plan.from_tensors([Wd], [Gd], [Md], Th, Tw_per_layer=[Tw]).bind()
+    plan.step(hp)
+    torch.cuda.synchronize()
+    Wr, Mr, Ur = PU.O.step_rect(PU.f64(W0), PU.f64(G), PU.f64(M), PU.oracle_hp(hp), Th, Tw)
+    m_gpu, w_gpu = PU.f64(Md.cpu()), PU.f64(Wd.cpu())
+    assert np.all(np.abs(m_gpu - Mr) <= PU.BF16_ULP * np.abs(Mr) + 2.0 ** -21 * (np.abs(0.95 * PU.f64(M)) + np.abs(PU.f64(G))) + 1e-30)
+    tau = PU.O.tau_rect(H, W, Th, Tw, 0.2)
+    for r in range(H // Th):
+        for c in range(W // Tw):
+            sl = (slice(r * Th, (r + 1) * Th), slice(c * Tw, (c + 1) * Tw))
+            dW = np.linalg.norm(w_gpu[sl] - Wr[sl])
+            bound = PU.BF16_ULP * np.linalg.norm(Wr[sl]) + 0.02 * tau * PU.TOL_TC * np.linalg.norm(Ur[sl])
+            assert dW <= bound, f"tile ({r},{c}): {dW / bound:.3f}"

@@ -197,3 +197,19 @@ def test_kernel_paths_bucket_the_work_list():
     assert p.n_tiles == 256 + 64 + 16 + 4 + 1 + 4
     _, offs, cT = p.worklist()
     assert cT.tolist() == [16, 32, 64, 128, 256, 128] and p.n_chunks == 6
+
+
+def test_rectangular_tiles_plan():
+    """T_w != T: R = ceil(H/T), C = ceil(W/T_w), both extents powers of two in 16..2048."""
+    L = [hm.himuon_layer(hm.shape_mat(300, 500), hm.shape_mat(300, 500), hm.shape_mat(300, 500), 128, 32)]
+    p = hm.Plan(L, 128)
+    lrc, _, cT = p.worklist()
+    assert p.n_tiles == 3 * 16 and lrc[-1].tolist() == [0, 2, 15] and cT.tolist() == [128]
+    L[0].T_w = 128                                   # T_w == T is the square case: tensor-core kernel, no scratch
+    assert hm.Plan(L, 128).workspace_bytes < 1 << 20
+    L[0].T_w = 48
+    with pytest.raises(hm.HimuonError) as e:
+        hm.Plan(L, 128)
+    assert e.value.status == B.HIMUON_ERR_INVALID_ARG
+    L[0].T, L[0].T_w = 512, 1024                     # one tile covers the matrix: full-matrix branch
+    assert hm.Plan(L, 128).n_tiles == 1

@@ -278,7 +278,7 @@ def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
     pipelined over three streams so that the copies of one group overlap the step of another (PCIe is full
     duplex).  Host buffers are bounded by --e2e-host-gb."""
     sizes = [g.numel() * 2 for g in Gs]
-    budget = int(args.e2e_host_gb * (1 << 30))
+    budget = int(args.e2e_host_gb * (1 << 30) / max(1, world))   # pinned host memory is shared by the ranks of a node
     n_layers, acc = 0, 0
     for sz in sizes:                       # both a G-in and a W-out host buffer per layer
         if acc + 2 * sz > budget:

@@ -146,7 +146,11 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   // which: 1 = MMA1 (B = XB, K-major), 2 = MMA2 (B = OB, K-major), 3 = MMA3 (B = Xb copy in ST, MN-major).
   auto ready_and_issue = [&](int which) {
     tmem_wait_st();
-    fence_proxy_async_all();          // generic-proxy writes (local and remote smem) -> visible to the MMA
+    // generic-proxy writes -> visible to the MMA.  Remote (DSMEM) writes happen only in write_xb_copy, between the
+    // issue of MMA1 and this call for MMA2, so only that call needs the fence over all state spaces.
+    // The phase before MMA3 writes tensor memory only.
+    if (which == 2) fence_proxy_async_all();
+    else if (which == 1) fence_proxy_async_smem();
     tc_fence_before_sync();
     __syncthreads();
     if (lead) {

@@ -213,3 +213,26 @@ def test_rectangular_tiles_plan():
     assert e.value.status == B.HIMUON_ERR_INVALID_ARG
     L[0].T, L[0].T_w = 512, 1024                     # one tile covers the matrix: full-matrix branch
     assert hm.Plan(L, 128).n_tiles == 1
+
+
+def test_chunk_rule_properties():
+    """Properties of the memory-bounded chunk rule (fewest chunks that fit, balanced sizes)
+    over random instances, against what the rule must guarantee rather than against a second implementation."""
+    from hypothesis import given, settings, strategies as st
+
+    @settings(max_examples=300, deadline=None)
+    @given(n=st.integers(0, 200000), per=st.integers(1, 1 << 20), fixed=st.integers(0, 1 << 20), slack=st.integers(0, 1 << 24))
+    def check(n, per, fixed, slack):
+        cap = fixed + per + slack                       # room for at least one item
+        offs = hm.himuon_plan_chunks(n, per, fixed, cap)
+        assert offs[0] == 0 and offs[-1] == n and all(b > a for a, b in zip(offs, offs[1:]))
+        sizes = np.diff(offs)
+        if n == 0:
+            assert len(offs) == 1
+            return
+        per_max = (cap - fixed) // per
+        assert sizes.max() <= per_max                    # every chunk fits under the cap
+        assert len(sizes) == -(-n // per_max)            # and there are as few chunks as that allows
+        assert sizes.max() - sizes.min() <= 1            # balanced (5376 -> 2 x 2688)
+
+    check()

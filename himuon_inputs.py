@@ -200,3 +200,41 @@ def make_param_set(spec: ParamSetSpec, *, dtype=torch.bfloat16, device="cpu",
         W, G, M = make_layer_tensors(spec, i, dtype=dtype, device=device)
         Ws.append(W); Gs.append(G); Ms.append(M)
     return Ws, Gs, Ms
+
+
+# ----------------------------------------------------------------------------- capacity diagnostic workload
+# The one-step linear associative-memory benchmark the paper uses as its capacity diagnostic
+# (section 5.1; instance sizes PAPER.md:410 section 6.5).  This is the WORKLOAD around
+# the map - key/value embeddings, the minibatch, the gradient of the cross-entropy loss at W_0 = 0 and the
+# recovered-item count - and holds none of the method's arithmetic: the update map is applied by the
+# caller (the oracle in the CPU pins, the CUDA path in the GPU tests).
+
+@dataclass
+class AssocMemoryProblem:
+    U: np.ndarray          # [N, d] values u_j  ~ N(0, I/d)
+    V: np.ndarray          # [N, d] keys   v_i  ~ N(0, I/d)
+    idx: np.ndarray        # [B] sampled item indices, p_i ~ i^-alpha (with replacement)
+    G0: np.ndarray         # [d, d] minibatch gradient of the cross-entropy loss at W_0 = 0, float64
+
+
+def assoc_memory_problem(d: int, N: int, alpha: float, B: int, seed: int) -> AssocMemoryProblem:
+    """Logits of key v_i are u_j^T W v_i; at W_0 = 0 the softmax is uniform, so the
+    gradient of the mean cross-entropy over the minibatch is
+        G_0 = (1/B) sum_b (ubar - u_{i_b}) v_{i_b}^T,   ubar = (1/N) sum_j u_j,
+    built in float64 (PAPER.md:410 "constructed in fp64 and held fixed across precision variants")."""
+    g = np.random.default_rng(1_000_003 * 7 + seed)
+    V = g.standard_normal((N, d)) / math.sqrt(d)
+    U = g.standard_normal((N, d)) / math.sqrt(d)
+    p = np.arange(1, N + 1, dtype=np.float64) ** (-alpha)
+    p /= p.sum()
+    idx = g.choice(N, size=B, p=p)
+    cnt = np.bincount(idx, minlength=N).astype(np.float64)
+    ubar = U.mean(axis=0)
+    G0 = ((cnt[:, None] * (ubar[None, :] - U)).T @ V) / B
+    return AssocMemoryProblem(U=U, V=V, idx=idx, G0=G0)
+
+
+def recovered_items(prob: AssocMemoryProblem, W1: np.ndarray) -> int:
+    """Number of items k with argmax_j u_j^T W_1 v_k = k."""
+    logits = (prob.U @ W1) @ prob.V.T          # [j, k]
+    return int((np.argmax(logits, axis=0) == np.arange(prob.U.shape[0])).sum())

@@ -28,3 +28,8 @@ def read_golden(name):
 @pytest.fixture(scope="session")
 def paper_numbers():
     return read_golden("paper_planner_numbers.txt")
+
+
+@pytest.fixture(scope="session")
+def paper_table3():
+    return read_golden("paper_table3_recovered_items.txt")

@@ -182,7 +182,8 @@ def run_gpu(args):
         spec.layers = [spec.layers[i] for i in mine]
     Ws, Gs, Ms = make_inputs(spec, dev)                       # default (weak scaling): every rank owns a full parameter set
     Tl = [l.T for l in spec.layers]
-    plan = hm.Plan.from_tensors(Ws, Gs, Ms, args.T, T_per_layer=Tl if any(Tl) else None,
+    path = hm.HIMUON_PATH_FP8 if args.path == "fp8" else hm.HIMUON_PATH_AUTO
+    plan = hm.Plan.from_tensors(Ws, Gs, Ms, args.T, T_per_layer=Tl if any(Tl) else None, path=path,
                                 workspace_cap_bytes=args.cap_mb << 20).bind()
     flops = algorithmic_flops(spec, args.T, args.K)
     n_elem = spec.n_elements
@@ -234,6 +235,10 @@ def run_gpu(args):
     # dominant kernel = the fused step kernel of the plan-wide tile size (one launch per chunk)
     kname = {16: "himuon_warp_kernel", 32: "himuon_warp_kernel", 64: "himuon_tc64_kernel", 128: "himuon_tc128_kernel",
              256: "himuon_tc256_kernel"}.get(args.T, "himuon_simt_kernel")
+    if args.path == "fp8":                                    # e4m3 peak = measured bf16 peak x the nominal 2:1 ratio
+        kname = "himuon_tc128_fp8_kernel"
+        pk = dict(pk, bf16_sustained=2 * pk["bf16_sustained"], bf16_burst=2 * pk["bf16_burst"],
+                  source=pk["source"] + " x2 (nominal fp8:bf16 ratio)")
     kern_ms = statistics.mean(per_step) / max(1, plan.n_chunks)
     bytes_step = 10.0 * n_elem
     t_tensor = flops / (pk["bf16_sustained"] * 1e12)
@@ -261,7 +266,7 @@ def run_gpu(args):
     cpu = run_cpu_baseline(args, spec, hp)
     line = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
-            "scaling": "strong" if args.shard else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "scaling": "strong" if args.shard else "weak", "vs_baseline": None, "dtype": "fp8-e4m3 operands, fp32 state" if args.path == "fp8" else "bf16", "data": "synthetic",
             "config": {"workload": f"{spec.name}-shaped HiMuon step (BASELINE configs[4])" if spec.name.startswith("llama3-8b") else f"{spec.name}-shaped HiMuon step",
                        "layers": len(spec.layers), "elements": n_elem, "tiles": plan.n_tiles, "T": args.T, "K": args.K,
                        "chunks": plan.n_chunks, "workspace_bytes": plan.workspace_bytes, "cap_mb": args.cap_mb,
@@ -294,7 +299,8 @@ def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
     for gr in groups:
         Ms_g = [torch.zeros_like(Gs[i]) for i in gr]
         plans.append(hm.Plan.from_tensors([Ws[i] for i in gr], [Gs[i] for i in gr], Ms_g, args.T,
-                                          T_per_layer=[Tl[i] for i in gr] if any(Tl) else None).bind())
+                                          T_per_layer=[Tl[i] for i in gr] if any(Tl) else None,
+                                          path=hm.HIMUON_PATH_FP8 if args.path == "fp8" else hm.HIMUON_PATH_AUTO).bind())
     sub_flops = float(sum(6.0 * args.K * (spec.layers[i].T or args.T) * spec.layers[i].H * spec.layers[i].W for i in range(n_layers)))
     hG = [torch.empty(Gs[i].shape, dtype=Gs[i].dtype, pin_memory=True) for i in range(n_layers)]
     hW = [torch.empty(Ws[i].shape, dtype=Ws[i].dtype, pin_memory=True) for i in range(n_layers)]
@@ -400,6 +406,8 @@ def main():
     ap.add_argument("--workload", default="llama3-8b")
     ap.add_argument("--T", type=int, default=128)
     ap.add_argument("--K", type=int, default=5)
+    ap.add_argument("--path", default="auto", choices=["auto", "fp8"],
+                    help="fp8: e4m3 operands in the Newton-Schulz products (T = 128 only; NOT the headline: reduced precision)")
     ap.add_argument("--cap-mb", type=int, default=2048)
     ap.add_argument("--cpu-tiles", type=int, default=16384)
     ap.add_argument("--e2e-host-gb", type=float, default=8.0)

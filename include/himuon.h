@@ -61,8 +61,14 @@ typedef enum { HIMUON_F32 = 0, HIMUON_BF16 = 1 } himuon_dtype;
  *          the large-tile path at T = 256;
  *          fp32 storage -> fp32 path.
  *   FP32 : true fp32 arithmetic for any storage dtype: FMA kernel for T in {16, 32, 64, 128}, the large-tile
- *          path with true-fp32 cuBLAS products for T = 256, 512 and the full-matrix branch (the <= 1e-4 path). */
-typedef enum { HIMUON_PATH_AUTO = 0, HIMUON_PATH_FP32 = 1 } himuon_path;
+ *          path with true-fp32 cuBLAS products for T = 256, 512 and the full-matrix branch (the <= 1e-4 path).
+ *   FP8  : bf16 storage, T = 128, width a multiple of 8 only (anything else: HIMUON_ERR_UNSUPPORTED).  The three
+ *          products of a Newton-Schulz step take e4m3 operands (tcgen05 kind::f8f6f4, fp32 accumulation); the
+ *          iterate, the diagonals of A and B, momentum and update stay fp32.  Opt-in:
+ *          per-tile error about 0.1 instead of <= 3e-2 on Gaussian-like and low-rank tiles, and a heavy-tailed
+ *          tile dominated by a few entries (Student-t with 2 degrees of freedom) can leave the basin of the quintic:
+ *          the result is then finite but wrong by O(1) or more.  Never selected by AUTO. */
+typedef enum { HIMUON_PATH_AUTO = 0, HIMUON_PATH_FP32 = 1, HIMUON_PATH_FP8 = 2 } himuon_path;
 
 /* {ptr, H, W, ld, dtype}: one row-major device matrix. */
 typedef struct {

@@ -25,7 +25,7 @@ HIMUON_ERR_CUDA = 4
 HIMUON_ERR_NOT_BOUND = 5
 
 HIMUON_F32, HIMUON_BF16 = 0, 1
-HIMUON_PATH_AUTO, HIMUON_PATH_FP32 = 0, 1
+HIMUON_PATH_AUTO, HIMUON_PATH_FP32, HIMUON_PATH_FP8 = 0, 1, 2
 
 # PAPER.md:74 Eq. (2.3)
 NS_COEFFS = (3.4445, -4.7750, 2.0315)
@@ -102,6 +102,8 @@ def _lib():
     lib.himuon_launch_count.argtypes = []
     lib.himuon_debug_set_tc128_stage.restype = None
     lib.himuon_debug_set_tc128_stage.argtypes = [C.c_int]
+    lib.himuon_debug_set_tc128_fp8_stage.restype = None
+    lib.himuon_debug_set_tc128_fp8_stage.argtypes = [C.c_int]
     _LIB = lib
     return lib
 
@@ -280,3 +282,7 @@ def himuon_ns_tiles(tiles_in: torch.Tensor, tiles_out: Optional[torch.Tensor] = 
 
 def debug_set_tc128_stage(stage: int):
     _lib().himuon_debug_set_tc128_stage(stage)
+
+
+def debug_set_tc128_fp8_stage(stage: int):
+    _lib().himuon_debug_set_tc128_fp8_stage(stage)

@@ -33,6 +33,8 @@ const int kTileSizes[] = {16, 32, 64, 128, 256, 512};
 // of the last granule, i.e. it would write into the ld - W gutter).
 int select_kpath(int dtype, int path, int T, int W = 0) {
   const bool simt_ok = (T == 16 || T == 32 || T == 64 || T == 128);
+  if (path == HIMUON_PATH_FP8)                                      // e4m3 operands: the T = 128 tcgen05 kernel only
+    return (dtype == HIMUON_BF16 && T == 128 && (W % 8) == 0) ? KPATH_TC_FP8 : -1;
   if (T >= 512) return KPATH_GEMM;                                  // library-size products: cuBLAS
   if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : (T == 256 ? KPATH_GEMM : -1);
   // bf16 storage, AUTO: tensor-core path where it exists, else the fp32 kernel / the large-tile path.
@@ -116,6 +118,7 @@ himuon_status chunk_rule(long long n_items, long long bytes_per_item, long long 
 
 cudaError_t launch_chunk(const LaunchArgs& a, int kpath, cudaStream_t s) {
   g_launches.fetch_add(1);
+  if (kpath == KPATH_TC_FP8) return launch_tc128_fp8(a, s);
   if (kpath == KPATH_TC) return a.T == 64 ? launch_tc64(a, s) : a.T == 256 ? launch_tc256(a, s) : launch_tc128(a, s);
   if (kpath == KPATH_WARP) return launch_warp(a, s);
   return launch_simt(a, s);
@@ -181,7 +184,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
   if (!out) return HIMUON_ERR_INVALID_ARG;
   *out = nullptr;
   if (!layers || n_layers <= 0) return HIMUON_ERR_INVALID_ARG;
-  if (path != HIMUON_PATH_AUTO && path != HIMUON_PATH_FP32) return HIMUON_ERR_INVALID_ARG;
+  if (path != HIMUON_PATH_AUTO && path != HIMUON_PATH_FP32 && path != HIMUON_PATH_FP8) return HIMUON_ERR_INVALID_ARG;
   if (T_default < 0) return HIMUON_ERR_INVALID_ARG;
 
   himuon_plan* p = new (std::nothrow) himuon_plan();
@@ -223,6 +226,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       if (select_kpath(dt, path, T) < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
       Te = T;
     }
+    if (rect && path == HIMUON_PATH_FP8) { st = HIMUON_ERR_UNSUPPORTED; break; }   // e4m3 operands: square T = 128 only
     const int kp = rect ? KPATH_GEMM : select_kpath(dt, path, Te, W);
     if (kp < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
     if (!rect) Twe = Te;
@@ -248,7 +252,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
     p->kpath[l] = kp;
     if (!L.g.ptr || !L.w.ptr) p->bindable = false;
     const size_t esz = dt == HIMUON_BF16 ? 2 : 4;
-    if (kp == KPATH_TC) {
+    if (kpath_uses_tma(kp)) {
       p->needs_tma = true;
       const himuon_mat* ms[3] = {&L.w, &L.g, &L.m};
       for (int i = 0; i < 3; ++i) {
@@ -369,7 +373,7 @@ himuon_status himuon_plan_bind(himuon_plan* plan, void* workspace, size_t worksp
     std::vector<CUtensorMap> maps((size_t)n * 3);
     std::memset(maps.data(), 0, maps.size() * sizeof(CUtensorMap));
     for (int l = 0; l < n; ++l) {
-      if (plan->kpath[l] != KPATH_TC) continue;
+      if (!kpath_uses_tma(plan->kpath[l])) continue;
       const himuon_layer& L = plan->layers[l];
       const himuon_mat*   ms[3] = {&L.w, &L.g, &L.m};
       for (int i = 0; i < 3; ++i) {
@@ -458,7 +462,7 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
                               float eps, void* workspace, size_t workspace_bytes, void* cuda_stream) {
   if (n_tiles < 0) return HIMUON_ERR_INVALID_ARG;
   if (dtype != HIMUON_F32 && dtype != HIMUON_BF16) return HIMUON_ERR_INVALID_ARG;
-  if (path != HIMUON_PATH_AUTO && path != HIMUON_PATH_FP32) return HIMUON_ERR_INVALID_ARG;
+  if (path != HIMUON_PATH_AUTO && path != HIMUON_PATH_FP32 && path != HIMUON_PATH_FP8) return HIMUON_ERR_INVALID_ARG;
   bool known = false;
   for (int t : kTileSizes) known |= (t == T);
   if (!known) return HIMUON_ERR_INVALID_ARG;
@@ -474,7 +478,7 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
   if (workspace_bytes < himuon_ns_tiles_workspace_bytes()) return HIMUON_ERR_WORKSPACE_TOO_SMALL;
   if ((uintptr_t)workspace & 127) return HIMUON_ERR_INVALID_ARG;
   const size_t esz = dtype == HIMUON_BF16 ? 2 : 4;
-  if (kp == KPATH_TC && (((uintptr_t)tiles_in & 15) || ((uintptr_t)tiles_out & 15))) return HIMUON_ERR_UNSUPPORTED;
+  if (kpath_uses_tma(kp) && (((uintptr_t)tiles_in & 15) || ((uintptr_t)tiles_out & 15))) return HIMUON_ERR_UNSUPPORTED;
   if (((uintptr_t)tiles_in & (esz - 1)) || ((uintptr_t)tiles_out & (esz - 1))) return HIMUON_ERR_INVALID_ARG;
 
   // The packed batch is one (n_tiles*T) x T matrix whose tile (r, 0) is tile r.
@@ -499,7 +503,7 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
   }
   cudaError_t e = cudaMemcpyAsync(ws, &D, sizeof(D), cudaMemcpyHostToDevice, s);
   if (e != cudaSuccess) return cuda_fail(e, "ns_tiles: layer table");
-  if (kp == KPATH_TC) {
+  if (kpath_uses_tma(kp)) {
     CUtensorMap maps[3];
     std::memset(maps, 0, sizeof(maps));
     if (!encode_bf16_map(&maps[0], D.w, D.H, D.W, T, T > 128 ? 128 : T) || !encode_bf16_map(&maps[1], D.g, D.H, D.W, T, T > 128 ? 128 : T)) {

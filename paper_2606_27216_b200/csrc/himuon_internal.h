@@ -34,7 +34,8 @@ struct WorkItem {
 static_assert(sizeof(WorkItem) == 16, "WorkItem must be 16 bytes");
 
 enum Mode : int { MODE_STEP = 0, MODE_PHI = 1 };
-enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1, KPATH_WARP = 2, KPATH_GEMM = 3 };
+enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1, KPATH_WARP = 2, KPATH_GEMM = 3, KPATH_TC_FP8 = 4 };
+inline bool kpath_uses_tma(int kp) { return kp == KPATH_TC || kp == KPATH_TC_FP8; }
 constexpr int kWholeMatrixT = 1 << 20;   // tile size of the full-matrix branch beyond the largest tile kernel (R = C = 1)
 
 struct LaunchArgs {
@@ -52,6 +53,7 @@ struct LaunchArgs {
 cudaError_t launch_simt(const LaunchArgs& a, cudaStream_t stream);
 // kernels_tc128.cu -- tcgen05 bf16 path, T = 128, bf16 storage.
 cudaError_t launch_tc128(const LaunchArgs& a, cudaStream_t stream);
+cudaError_t launch_tc128_fp8(const LaunchArgs& a, cudaStream_t stream);   // e4m3 operands, HIMUON_PATH_FP8
 // kernels_tc64.cu -- tcgen05 bf16 path, T = 64 (two tiles stacked per MMA), bf16 storage.
 cudaError_t launch_tc64(const LaunchArgs& a, cudaStream_t stream);
 // kernels_tc256.cu -- tcgen05 cta_group::2 bf16 path, T = 256 (one tile per CTA pair), bf16 storage.

@@ -236,3 +236,21 @@ def test_chunk_rule_properties():
         assert sizes.max() - sizes.min() <= 1            # balanced (5376 -> 2 x 2688)
 
     check()
+
+
+def test_fp8_path_is_opt_in_and_T128_only():
+    """HIMUON_PATH_FP8 (e4m3 operands, include/himuon.h): bf16 storage, T = 128, width a multiple of 8 - everything
+    else is refused at plan time, never silently served by another kernel; AUTO never selects it."""
+    U = B.HIMUON_ERR_UNSUPPORTED
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16, hm.HIMUON_PATH_FP8) == [128]
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_F32, hm.HIMUON_PATH_FP8) == []
+    p = hm.Plan(_layers([(512, 768), (100, 128)]), 128, path=hm.HIMUON_PATH_FP8)
+    assert p.n_tiles == 24 + 1 and p.n_buckets == 1
+    for shapes, T, kw in (([(512, 512)], 64, {}), ([(512, 512)], 256, {}), ([(512, 512)], 512, {}),
+                          ([(512, 500)], 128, {}), ([(512, 512)], 128, {"dtype": hm.HIMUON_F32})):
+        with pytest.raises(hm.HimuonError) as e:
+            hm.Plan(_layers(shapes, **kw), T, path=hm.HIMUON_PATH_FP8)
+        assert e.value.status == U, (shapes, T, kw)
+    with pytest.raises(hm.HimuonError) as e:                    # an unknown path value is an argument error
+        hm.Plan(_layers([(256, 256)]), 128, path=3)
+    assert e.value.status == B.HIMUON_ERR_INVALID_ARG

@@ -45,7 +45,7 @@ def _cut(t, T, r, c):
     return t[r * T:(r + 1) * T, c * T:(c + 1) * T].clone()
 
 
-def _run_config_step(spec, T_default, cap_mb, n_sample, seed):
+def _run_config_step(spec, T_default, cap_mb, n_sample, seed, path=hm.HIMUON_PATH_AUTO, tol=PU.TOL_TC):
     hp = hm.HParams(K=5, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
     Tl = [l.T or T_default for l in spec.layers]
     Ws, Gs, Ms = [], [], []
@@ -56,7 +56,7 @@ def _run_config_step(spec, T_default, cap_mb, n_sample, seed):
     before = [(_cut(Ws[li], Tl[li], r, c).cpu(), _cut(Gs[li], Tl[li], r, c).cpu(), _cut(Ms[li], Tl[li], r, c).cpu())
               for (li, r, c) in picks]
     plan = hm.Plan.from_tensors(Ws, Gs, Ms, T_default, T_per_layer=Tl if any(l.T for l in spec.layers) else None,
-                                workspace_cap_bytes=cap_mb << 20).bind()
+                                path=path, workspace_cap_bytes=cap_mb << 20).bind()
     plan.step(hp)
     torch.cuda.synchronize()
     worst = 0.0
@@ -69,7 +69,7 @@ def _run_config_step(spec, T_default, cap_mb, n_sample, seed):
             out = torch.zeros(T, T, dtype=x.dtype)
             out[:x.shape[0], :x.shape[1]] = x
             return out
-        ratio = PU.check_step(pad(W0), pad(G0), pad(M0), pad(W1), pad(M1), T, hp, PU.TOL_TC, storage_bf16=True)
+        ratio = PU.check_step(pad(W0), pad(G0), pad(M0), pad(W1), pad(M1), T, hp, tol, storage_bf16=True)
         worst = max(worst, ratio)
     return plan, worst, len(picks)
 
@@ -96,6 +96,36 @@ def test_config5_llama3_8b_step(T):
     plan, worst, n = _run_config_step(I.llama3_8b_spec(), T, 2048, 128, 5)
     assert plan.n_tiles == {128: 425984, 64: 1703936, 256: 106496, 32: 6815744, 16: 27262976}[T]
     assert plan.workspace_bytes <= 2048 << 20
+
+
+def test_config5_llama3_8b_step_fp8():
+    """The same full-size launch on the opt-in e4m3-operand path (HIMUON_PATH_FP8), at its own tolerance (0.15)."""
+    _need_gpu(120)
+    plan, worst, n = _run_config_step(I.llama3_8b_spec(), 128, 2048, 128, 5, path=hm.HIMUON_PATH_FP8, tol=0.15)
+    assert plan.n_tiles == 425984
+
+
+def test_config4_gpt2_xl_ragged_fp8_deterministic():
+    """GPT-2-XL shapes (64-wide edge tiles) on the e4m3-operand path: two steps from the same bits twice give bitwise
+    identical W' and M' (no race between the slots, the prefetches and the stores)."""
+    _need_gpu(40)
+    spec = I.gpt2_xl_spec(n_blocks=4)
+    hp = hm.HParams(K=5, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
+    outs = []
+    for rep in range(2):
+        Ws, Gs, Ms = [], [], []
+        for i in range(len(spec.layers)):
+            W, G, M = I.make_layer_tensors(spec, i, dtype=torch.bfloat16, device=DEV)
+            Ws.append(W); Gs.append(G); Ms.append(M)
+        plan = hm.Plan.from_tensors(Ws, Gs, Ms, 128, path=hm.HIMUON_PATH_FP8).bind()
+        plan.step(hp)
+        plan.step(hp)
+        torch.cuda.synchronize()
+        outs.append((Ws, Ms))
+        plan.destroy()
+    for a, b in zip(outs[0][0] + outs[0][1], outs[1][0] + outs[1][1]):
+        assert torch.equal(a, b)
+        assert bool(torch.isfinite(a.float()).all())
 
 
 def test_config5_schedule_per_layer_type():

@@ -62,7 +62,7 @@ typedef enum { HIMUON_F32 = 0, HIMUON_BF16 = 1 } himuon_dtype;
  *          fp32 storage -> fp32 path.
  *   FP32 : true fp32 arithmetic for any storage dtype: FMA kernel for T in {16, 32, 64, 128}, the large-tile
  *          path with true-fp32 cuBLAS products for T = 256, 512 and the full-matrix branch (the <= 1e-4 path).
- *   FP8  : bf16 storage, T = 128, width a multiple of 8 only (anything else: HIMUON_ERR_UNSUPPORTED).  The three
+ *   FP8  : bf16 storage, T = 128 or 256, width a multiple of 8 only (anything else: HIMUON_ERR_UNSUPPORTED).  The three
  *          products of a Newton-Schulz step take e4m3 operands (tcgen05 kind::f8f6f4, fp32 accumulation); the
  *          iterate, the diagonals of A and B, momentum and update stay fp32.  Opt-in:
  *          per-tile error about 0.1 instead of <= 3e-2 on Gaussian-like and low-rank tiles, and a heavy-tailed

@@ -18,7 +18,7 @@ CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libhimuon.so")
 STAMP_PATH = os.path.join(PKG_DIR, "libhimuon.stamp")
 
-SOURCES = ["himuon_api.cu", "kernels_simt.cu", "kernels_tc128.cu", "kernels_tc128_fp8.cu", "kernels_tc64.cu", "kernels_tc256.cu", "kernels_warp.cu", "kernels_gemm.cu"]
+SOURCES = ["himuon_api.cu", "kernels_simt.cu", "kernels_tc128.cu", "kernels_tc128_fp8.cu", "kernels_tc64.cu", "kernels_tc256.cu", "kernels_tc256_fp8.cu", "kernels_warp.cu", "kernels_gemm.cu"]
 HEADERS = ["himuon_internal.h", "sm100_ptx.cuh", "tc_common.cuh", os.path.join(ROOT, "include", "himuon.h")]
 
 NVCC_FLAGS = [

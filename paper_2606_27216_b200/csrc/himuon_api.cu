@@ -33,8 +33,8 @@ const int kTileSizes[] = {16, 32, 64, 128, 256, 512};
 // of the last granule, i.e. it would write into the ld - W gutter).
 int select_kpath(int dtype, int path, int T, int W = 0) {
   const bool simt_ok = (T == 16 || T == 32 || T == 64 || T == 128);
-  if (path == HIMUON_PATH_FP8)                                      // e4m3 operands: the T = 128 tcgen05 kernel only
-    return (dtype == HIMUON_BF16 && T == 128 && (W % 8) == 0) ? KPATH_TC_FP8 : -1;
+  if (path == HIMUON_PATH_FP8)                                      // e4m3 operands: the T = 128 / 256 tcgen05 kernels only
+    return (dtype == HIMUON_BF16 && (T == 128 || T == 256) && (W % 8) == 0) ? KPATH_TC_FP8 : -1;
   if (T >= 512) return KPATH_GEMM;                                  // library-size products: cuBLAS
   if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : (T == 256 ? KPATH_GEMM : -1);
   // bf16 storage, AUTO: tensor-core path where it exists, else the fp32 kernel / the large-tile path.
@@ -118,7 +118,7 @@ himuon_status chunk_rule(long long n_items, long long bytes_per_item, long long 
 
 cudaError_t launch_chunk(const LaunchArgs& a, int kpath, cudaStream_t s) {
   g_launches.fetch_add(1);
-  if (kpath == KPATH_TC_FP8) return launch_tc128_fp8(a, s);
+  if (kpath == KPATH_TC_FP8) return a.T == 256 ? launch_tc256_fp8(a, s) : launch_tc128_fp8(a, s);
   if (kpath == KPATH_TC) return a.T == 64 ? launch_tc64(a, s) : a.T == 256 ? launch_tc256(a, s) : launch_tc128(a, s);
   if (kpath == KPATH_WARP) return launch_warp(a, s);
   return launch_simt(a, s);
@@ -226,7 +226,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       if (select_kpath(dt, path, T) < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
       Te = T;
     }
-    if (rect && path == HIMUON_PATH_FP8) { st = HIMUON_ERR_UNSUPPORTED; break; }   // e4m3 operands: square T = 128 only
+    if (rect && path == HIMUON_PATH_FP8) { st = HIMUON_ERR_UNSUPPORTED; break; }   // e4m3 operands: square tiles only
     const int kp = rect ? KPATH_GEMM : select_kpath(dt, path, Te, W);
     if (kp < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
     if (!rect) Twe = Te;

@@ -54,6 +54,7 @@ cudaError_t launch_simt(const LaunchArgs& a, cudaStream_t stream);
 // kernels_tc128.cu -- tcgen05 bf16 path, T = 128, bf16 storage.
 cudaError_t launch_tc128(const LaunchArgs& a, cudaStream_t stream);
 cudaError_t launch_tc128_fp8(const LaunchArgs& a, cudaStream_t stream);   // e4m3 operands, HIMUON_PATH_FP8
+cudaError_t launch_tc256_fp8(const LaunchArgs& a, cudaStream_t stream);
 // kernels_tc64.cu -- tcgen05 bf16 path, T = 64 (two tiles stacked per MMA), bf16 storage.
 cudaError_t launch_tc64(const LaunchArgs& a, cudaStream_t stream);
 // kernels_tc256.cu -- tcgen05 cta_group::2 bf16 path, T = 256 (one tile per CTA pair), bf16 storage.

@@ -93,29 +93,6 @@ __device__ __forceinline__ void issue_bx(uint32_t acc, uint32_t opa, uint32_t ti
   umma_commit(bar);
 }
 
-// four fp32 (two packed pairs) -> four e4m3 bytes, element 0 in the low byte
-__device__ __forceinline__ uint32_t cvt_e4m3x4(f2 v01, f2 v23) {
-  float a, b, c, d;
-  upk2(v01, a, b);
-  upk2(v23, c, d);
-  uint32_t r;
-  asm("{\n\t.reg .b16 lo, hi;\n\tcvt.rn.satfinite.e4m3x2.f32 lo, %2, %1;\n\tcvt.rn.satfinite.e4m3x2.f32 hi, %4, %3;\n\t"
-      "mov.b32 %0, {lo, hi};\n\t}"
-      : "=r"(r) : "f"(a), "f"(b), "f"(c), "f"(d));
-  return r;
-}
-// 16 accumulator columns, scaled by k -> 16 e4m3 (4 words)
-__device__ __forceinline__ void pack16_e4m3(const uint32_t (&r)[16], f2 k2, uint32_t (&p)[4]) {
-#pragma unroll
-  for (int j = 0; j < 4; ++j)
-    p[j] = cvt_e4m3x4(mul2(pk2u(r[4 * j], r[4 * j + 1]), k2), mul2(pk2u(r[4 * j + 2], r[4 * j + 3]), k2));
-}
-// Replace one byte of a packed 16-column chunk: word `idx` (0..3, or 4 for none) becomes (word & keep) | val.
-__device__ __forceinline__ void set_one4(uint32_t (&p)[4], int idx, uint32_t keep, uint32_t val) {
-#pragma unroll
-  for (int j = 0; j < 4; ++j) p[j] = (j == idx) ? ((p[j] & keep) | val) : p[j];
-}
-
 __global__ void __launch_bounds__(kThreads, 1)
 himuon_tc128_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __restrict__ tmaps,
                     const WorkItem* __restrict__ items, long long n_items, int mode, himuon_hparams hp, int dbg) {

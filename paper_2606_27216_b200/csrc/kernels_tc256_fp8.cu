@@ -1,0 +1,469 @@
+// fp8 (e4m3) variant of the T = 256 CTA-pair kernel (HIMUON_PATH_FP8).
+// Same structure and synchronisation as kernels_tc256.cu (read its header first): one 256 x 256 tile per CTA pair,
+// rows split over the two CTAs, every product one pair MMA with M = 256, N = 256, K = 256.  What changes is the
+// operand format of the three products of a Newton-Schulz step: e4m3 (tcgen05.mma kind::f8f6f4, K = 32 per
+// instruction: 8 instead of 16 MMAs per product, half the operand bytes in shared and tensor memory and through
+// distributed shared memory).  Accumulation, the iterate, the diagonals of A and B, momentum and update stay fp32.
+// Operand scales and their justification: header of kernels_tc128_fp8.cu (the bounds do not depend on T).
+#include <cuda_bf16.h>
+#include <stddef.h>
+
+#include "himuon_internal.h"
+#include "sm100_ptx.cuh"
+#include "tc_common.cuh"
+
+namespace himuon {
+
+#define TR() do { } while (0)
+
+namespace {
+
+using namespace ptx;
+using namespace tc;
+
+constexpr int T = 256;
+constexpr int kRows = 128;                       // rows of the tile per CTA
+constexpr int kThreads = 512;                    // 16 warps: 4 lane quadrants x 4 column quarters
+constexpr uint32_t kBlkBytes = kRows * 128;      // 16 KB: 128 rows x 64 columns bf16 (one swizzle span wide)
+constexpr uint32_t kBufBytes = 4 * kBlkBytes;    // 64 KB: 128 rows x 256 columns
+constexpr uint32_t kAtomBytes = T * 128;         // 32 KB: 256 K-rows x 128 N-columns (e4m3) of the MN-major operand
+constexpr float kSX = 256.f, kSO = 128.f, kSB = 128.f;   // operand scales (powers of two)
+constexpr uint32_t kCtrlBytes = 8192;
+constexpr uint32_t kSmemBytes = 3 * kBufBytes + kCtrlBytes + 1024;   // XB, OB, ST + control + alignment slack
+constexpr uint32_t kAccCol = 0, kOpaCol = 256;   // TMEM: ACC 256 columns (fp32), OPA 64 columns (e4m3 quads)
+
+struct Ctrl {
+  unsigned long long mma_bar;     // completion of a pair MMA (multicast commit), one per CTA
+  unsigned long long ready_bar;   // leader CTA only: both CTAs' operands are in place (2 arrivals)
+  unsigned long long ld_bar;      // TMA loads of G (and M)
+  unsigned long long w_bar;       // TMA load of W
+  float dpart[4][kRows];          // per column quarter: partial d_t = sum_j Xh_tj^2
+  float spart[4][kRows];          // per column quarter: partial sum_j ACC_tj^2
+  float red[16];
+  float peer_ss;                  // the other CTA's sum of squares of Ghat
+  uint32_t tmem_base;
+};
+static_assert(sizeof(Ctrl) <= kCtrlBytes, "control block too large");
+
+__device__ __forceinline__ uint32_t chunk_addr(uint32_t rowaddr, int c) { return rowaddr ^ ((uint32_t)c << 4); }
+
+// e4m3 K-major operand, this CTA's 128 rows x K = 256 bytes: two 128-byte-swizzled blocks of 128 rows;
+// k-step kk = 32 elements = 32 B inside block kk >> 2.
+__device__ __forceinline__ uint64_t desc_kmajor(uint32_t buf, int kk) {
+  return make_smem_desc_sw128(buf + (kk >> 2) * kBlkBytes + (kk & 3) * 32, 16, 1024);
+}
+// e4m3 MN-major operand, K = 256 rows x this CTA's 128 N-columns (128 B = one swizzle span); k-step = 32 rows.
+__device__ __forceinline__ uint64_t desc_mnmajor(uint32_t buf, int kk) {
+  return make_smem_desc_sw128(buf + kk * 4096, kAtomBytes, 1024);
+}
+__device__ __forceinline__ void issue_pair(uint32_t acc, uint32_t opa, uint32_t buf, bool mn_major, uint32_t bar) {
+  const uint32_t idesc = mn_major ? make_idesc_e4m3(T, T, 0, 1) : make_idesc_e4m3(T, T, 0, 0);
+#pragma unroll
+  for (int kk = 0; kk < T / 32; ++kk)
+    umma_f8_ts_pair(acc, opa + 8 * kk, mn_major ? desc_mnmajor(buf, kk) : desc_kmajor(buf, kk), idesc, kk ? 1u : 0u);
+  umma_commit_pair(bar, (uint16_t)3);
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __restrict__ tmaps,
+                    const WorkItem* __restrict__ items, long long n_items, int mode, himuon_hparams hp) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  Ctrl* ctrl = reinterpret_cast<Ctrl*>(smem_raw + (smem0 - smem_u32(smem_raw)) + 3 * kBufBytes);
+
+  const int tid = threadIdx.x;
+  const int warp = tid >> 5;
+  const int wq = warp & 3;             // TMEM lane quadrant of this warp
+  const int q4 = warp >> 2;            // column quarter
+  const int lane = tid & 31;
+  const int t = wq * 32 + lane;        // local row / TMEM lane
+  const uint32_t rank = cluster_ctarank();
+  const int R = (int)rank * kRows + t; // row of the tile
+  const bool lead = (tid == 0);
+  const bool step_mode = (mode == MODE_STEP);
+  // diagonal element (R, R): column quarter R >> 6, 16-column chunk (R & 63) >> 4 of it, packed word (R & 15) >> 2, byte R & 3
+  const bool own = (q4 == (int)(2 * rank) + (wq >> 1));            // warp-uniform
+  const int dq = (t & 63) >> 4, dword = (t & 15) >> 2;
+  const uint32_t dshift = (uint32_t)(t & 3) * 8u;
+  const uint32_t dkeep = ~(0xffu << dshift);
+
+  const uint32_t XB = smem0, OB = XB + kBufBytes, ST = OB + kBufBytes;
+  const uint32_t rowoff = (uint32_t)q4 * kBlkBytes + (uint32_t)t * 128u + ((uint32_t)(t & 7) << 4);
+  const uint32_t xrow = XB + rowoff, orow = OB + rowoff, srow = ST + rowoff;   // bf16 staging rows
+  // e4m3 operand rows (first 32 KB of XB / OB): K-span block q4 >> 1, this thread's 64 bytes = chunks 4(q4&1)..+3
+  const uint32_t row8 = (uint32_t)(q4 >> 1) * kBlkBytes + (uint32_t)t * 128u + ((uint32_t)((4 * (q4 & 1)) ^ (t & 7)) << 4);
+  const uint32_t xrow8 = XB + row8, orow8 = OB + row8;
+  // this thread's 64 columns of row R in the MN-major (column-split) copy of Xb, which lives in the staging
+  // buffer ST during the steps: CTA q4 >> 1, atom q4 & 1, K-row R
+  const uint32_t xt_local = ST + (uint32_t)R * 128u + ((uint32_t)((4 * (q4 & 1)) ^ (R & 7)) << 4);
+  const bool xt_is_local = ((uint32_t)(q4 >> 1) == rank);              // warp-uniform
+  const uint32_t xt_row = xt_is_local ? xt_local : mapa_shared(xt_local, (uint32_t)(q4 >> 1));
+  const uint32_t mma_bar = smem_u32(&ctrl->mma_bar);
+  const uint32_t ready_bar = smem_u32(&ctrl->ready_bar);
+  const uint32_t ready_bar_leader = mapa_shared(ready_bar, 0);
+  const uint32_t ld_bar = smem_u32(&ctrl->ld_bar);
+  const uint32_t w_bar = smem_u32(&ctrl->w_bar);
+
+  if (tid == 0) {
+    mbar_init(mma_bar, 1);
+    mbar_init(ready_bar, 2);
+    mbar_init(ld_bar, 2);   // arrive.expect_tx at issue + "staging buffer is free" arrive of the lead thread
+    mbar_init(w_bar, 1);
+    fence_mbar_init();
+  }
+  cluster_sync_all();                                   // barriers of both CTAs exist before anyone signals
+  if (warp == 0) tmem_alloc_pair<512>(smem_u32(&ctrl->tmem_base));
+  tc_fence_before_sync();
+  cluster_sync_all();
+  tc_fence_after_sync();
+  const uint32_t tmem_base = ctrl->tmem_base;
+  const uint32_t lane_off = (uint32_t)(wq * 32) << 16;
+  const uint32_t acc_t = tmem_base + lane_off + kAccCol + 64u * q4;   // this thread's 64 accumulator columns
+  const uint32_t opa_t = tmem_base + lane_off + kOpaCol + 16u * q4;   // this thread's 16 packed operand columns
+  const uint32_t ACCd = tmem_base + kAccCol, OPAd = tmem_base + kOpaCol;
+
+  uint32_t ph_mma = 0, ph_ld = 0, ph_w = 0, ph_ready = 0;
+  const float qs = sqrtf(sqrtf(hp.c));         // state Xh = c^(1/4) X, see kernels_tc128.cu
+  const float beta_h = hp.b / sqrtf(hp.c);
+
+  // Operands of the next pair MMA are written: tell the leader; the leader issues once both CTAs have.
+  // which: 1 = MMA1 (B = XB, K-major), 2 = MMA2 (B = OB, K-major), 3 = MMA3 (B = Xb copy in ST, MN-major).
+  auto ready_and_issue = [&](int which) {
+    tmem_wait_st();
+    // generic-proxy writes -> visible to the MMA.  Remote (DSMEM) writes happen only in write_xb_copy, between the
+    // issue of MMA1 and this call for MMA2, so only that call needs the fence over all state spaces.
+    // The phase before MMA3 writes tensor memory only.
+    if (which == 2) fence_proxy_async_all();
+    else if (which == 1) fence_proxy_async_smem();
+    tc_fence_before_sync();
+    __syncthreads();
+    if (lead) {
+      mbar_arrive_cluster(ready_bar_leader);
+      if (rank == 0) {
+        mbar_wait_cluster(ready_bar, ph_ready);
+        tc_fence_after_sync();
+        issue_pair(ACCd, OPAd, which == 1 ? XB : which == 2 ? OB : ST, which == 3, mma_bar);
+      }
+    }
+    ph_ready ^= 1;
+  };
+  auto wait_mma = [&]() {   // one warp polls, the others sleep on a hardware barrier
+    if (warp == 0) mbar_wait(mma_bar, ph_mma);
+    named_bar_sync(1, kThreads);
+    ph_mma ^= 1;
+    tc_fence_after_sync();
+  };
+
+  // The column-split bf16 copy of the iterate that MMA3 reads (into ST of the owning CTA).  Called right after
+  // MMA1 has been issued, i.e. off the critical path: the stores (half of them remote) overlap the MMA.
+  auto write_xb_copy = [&](const f2 (&xs)[32]) {
+    const f2 sx2 = pk2(kSX, kSX);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      uint32_t x8[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) x8[j] = cvt_e4m3x4(mul2(xs[8 * q + 2 * j], sx2), mul2(xs[8 * q + 2 * j + 1], sx2));
+      if (xt_is_local) sts128(chunk_addr(xt_row, q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
+      else st_cluster_v4(chunk_addr(xt_row, q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
+    }
+  };
+
+  // G -> OB and (step mode) M -> XB of tile i: this CTA's 128 rows, four 64-column boxes each
+  auto issue_gm = [&](long long i) {
+    WorkItem wn;
+    if (items) wn = items[i];
+    else { wn.layer = 0; wn.r = (int)i; wn.c = 0; wn.pad = 0; }
+    const int xn = wn.c * T, yn = wn.r * T + (int)rank * kRows;
+    mbar_arrive_expect_tx(ld_bar, step_mode ? 2 * kBufBytes : kBufBytes);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      tma_load_2d(OB + j * kBlkBytes, tmaps + 3 * wn.layer + 1, xn + 64 * j, yn, ld_bar);
+      if (step_mode) tma_load_2d(XB + j * kBlkBytes, tmaps + 3 * wn.layer + 2, xn + 64 * j, yn, ld_bar);
+    }
+  };
+  bool prefetched = false;   // every thread tracks it (uniform); only the lead thread issues
+
+  for (long long it = cluster_id_x(); it < n_items; it += cluster_count_x()) {
+    TR();   // tile start
+    WorkItem wi;
+    if (items) wi = items[it];
+    else { wi.layer = 0; wi.r = (int)it; wi.c = 0; wi.pad = 0; }
+    const float tau_base = layers[wi.layer].tau_base;
+    const CUtensorMap* map_w = tmaps + 3 * wi.layer + 0;
+    const CUtensorMap* map_m = tmaps + 3 * wi.layer + 2;
+    const int x0 = wi.c * T, y0 = wi.r * T + (int)rank * kRows;
+    bool w_issued = false;
+    const long long nxt = it + cluster_count_x();
+
+    // ---------------- P: load, momentum, normalise ---------------------------------------------------
+    if (lead) {
+      if (!prefetched) issue_gm(it);
+      tma_wait_group_read0();   // the previous tile's stores out of ST have been read: M' may be written into it
+      mbar_arrive(ld_bar);
+    }
+    mbar_wait(ld_bar, ph_ld);
+    ph_ld ^= 1;
+    prefetched = false;
+
+    f2 xs[32];                  // fp32 state: this thread's 64 columns of row R, as packed pairs
+    f2 ss2 = pk2(0.f, 0.f);
+    const f2 beta2 = pk2(hp.beta, hp.beta);
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      const uint4 gv = lds128(chunk_addr(orow, c));
+      const uint32_t gw[4] = {gv.x, gv.y, gv.z, gv.w};
+      if (step_mode) {
+        const uint4 mv = lds128(chunk_addr(xrow, c));
+        const uint32_t mw[4] = {mv.x, mv.y, mv.z, mv.w};
+        uint32_t mo[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const f2 g2 = pk2u(gw[e] << 16, gw[e] & 0xffff0000u);
+          const f2 m2 = fma2(beta2, pk2u(mw[e] << 16, mw[e] & 0xffff0000u), g2);   // M' = beta M + G
+          mo[e] = cvt_bf16x2(m2);
+          const f2 h2 = hp.nesterov ? fma2(beta2, m2, g2) : m2;                    // Ghat
+          ss2 = fma2(h2, h2, ss2);
+          xs[4 * c + e] = h2;
+        }
+        sts128(chunk_addr(srow, c), make_uint4(mo[0], mo[1], mo[2], mo[3]));
+      } else {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const f2 h2 = pk2u(gw[e] << 16, gw[e] & 0xffff0000u);
+          ss2 = fma2(h2, h2, ss2);
+          xs[4 * c + e] = h2;
+        }
+      }
+    }
+    float s0, s1;
+    upk2(ss2, s0, s1);
+    const float ss = s0 + s1;
+    float tot = ss;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    if (lane == 0) ctrl->red[warp] = tot;
+    fence_proxy_async_smem();          // M' in ST -> visible to the TMA store
+    __syncthreads();
+    float mine = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) mine += ctrl->red[i];
+    if (lead) {
+      if (step_mode) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tma_store_2d(map_m, x0 + 64 * j, y0, ST + j * kBlkBytes);
+        tma_commit_group();
+        tma_wait_group_read0();   // after the cluster barrier below, ST of BOTH CTAs may receive the Xb copy
+      }
+      st_cluster_f32(mapa_shared(smem_u32(&ctrl->peer_ss), rank ^ 1u), mine);   // Frobenius norm spans both CTAs
+    }
+    cluster_sync_all();
+    tot = mine + ctrl->peer_ss;
+    const float nrm = sqrtf(tot);
+    const float inv = nrm > 0.f ? qs / (nrm + hp.eps) : 0.f;   // Phi_K(0) = 0
+    ctrl->dpart[q4][t] = ss * inv * inv;                        // partial diag(Ah)_R in fp32
+    {
+      const f2 inv2 = pk2(inv, inv), sx2 = pk2(kSX, kSX);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        uint32_t p[4];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) xs[8 * q + j] = mul2(xs[8 * q + j], inv2);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) p[j] = cvt_e4m3x4(mul2(xs[8 * q + 2 * j], sx2), mul2(xs[8 * q + 2 * j + 1], sx2));
+        sts128(chunk_addr(xrow8, q), make_uint4(p[0], p[1], p[2], p[3]));
+        tmem_st4(opa_t + 4 * q, p);
+      }
+    }
+    TR();   // prologue compute done
+    if (hp.K > 0) ready_and_issue(1);
+    else __syncthreads();
+    TR();   // MMA1 issued
+    if (hp.K > 0) write_xb_copy(xs);
+    float di = (ctrl->dpart[0][t] + ctrl->dpart[1][t]) + (ctrl->dpart[2][t] + ctrl->dpart[3][t]);
+
+    // ---------------- K Newton-Schulz steps ---------------------------------------------------
+#pragma unroll 1
+    for (int k = 0; k < hp.K; ++k) {
+      const bool last = (k + 1 == hp.K);
+      // ---- E1: ACC = rows of Ah
+      wait_mma();
+      TR();   // MMA1 done
+      {
+        // Ot = offdiag(Ah) + diag(d + beta/2), rounded to bf16: offdiag(Ot Ot^T) = offdiag(beta Ah + Ah^2)
+        // ACC = s_X^2 Ah; operand scale s_O: Ot s_O = ACC s_O / s_X^2
+        const uint32_t dval = (cvt_e4m3x4(pk2(kSO * fmaf(0.5f, beta_h, di), 0.f), pk2(0.f, 0.f)) & 0xffu) << dshift;
+        const f2 k1 = pk2(kSO / (kSX * kSX), kSO / (kSX * kSX));
+        f2 Sa = pk2(0.f, 0.f), Sb = Sa;
+        uint32_t r[2][16];
+        tmem_ld16(acc_t, r[0]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          tmem_wait_ld();
+          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          uint32_t(&c)[16] = r[q & 1];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const f2 o01 = pk2u(c[4 * j], c[4 * j + 1]), o23 = pk2u(c[4 * j + 2], c[4 * j + 3]);
+            Sa = fma2(o01, o01, Sa);
+            Sb = fma2(o23, o23, Sb);
+          }
+          uint32_t p[4];
+          pack16_e4m3(c, k1, p);
+          if (own) set_one4(p, dq == q ? dword : 4, dkeep, dval);
+          sts128(chunk_addr(orow8, q), make_uint4(p[0], p[1], p[2], p[3]));
+          tmem_st4(opa_t + 4 * q, p);
+        }
+        float s0, s1;
+        upk2(add2(Sa, Sb), s0, s1);
+        const float us = 1.f / (kSX * kSX);
+        ctrl->spart[q4][t] = (s0 + s1) * (us * us);          // partial (Ah^2)_RR from the scaled accumulator
+      }
+      TR();   // E1 loop done
+      ready_and_issue(2);
+      TR();   // MMA2 issued
+      // a + B_RR, B_RR = beta d_R + (Ah^2)_RR
+      const float si = hp.a + fmaf(beta_h, di, (ctrl->spart[0][t] + ctrl->spart[1][t]) + (ctrl->spart[2][t] + ctrl->spart[3][t]));
+
+      // ---- E2: ACC = rows of B (off-diagonal)
+      wait_mma();
+      TR();   // MMA2 done
+      {
+        uint32_t r[2][16];
+        tmem_ld16(acc_t, r[0]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          tmem_wait_ld();
+          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          uint32_t p[4];
+          pack16_e4m3(r[q & 1], pk2(kSB / (kSO * kSO), kSB / (kSO * kSO)), p);   // ACC = s_O^2 B; operand Bb s_B
+          if (own) set_one4(p, dq == q ? dword : 4, dkeep, 0u);
+          tmem_st4(opa_t + 4 * q, p);
+        }
+      }
+      TR();   // E2 loop done
+      ready_and_issue(3);
+      TR();   // MMA3 issued
+
+      // ---- E3: Xh = (a + B_RR) Xh + offdiag(B) Xh
+      wait_mma();
+      TR();   // MMA3 done
+      if (last && nxt < n_items) {                           // XB and OB are free (every pair MMA has completed)
+        if (lead) issue_gm(nxt);
+        prefetched = true;
+      }
+      if (last && lead && step_mode) {                       // ... and so is ST: fetch W into it
+        mbar_arrive_expect_tx(w_bar, kBufBytes);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tma_load_2d(ST + j * kBlkBytes, map_w, x0 + 64 * j, y0, w_bar);
+        w_issued = true;
+      }
+      {
+        const f2 si2 = pk2(si, si), k3 = pk2(1.f / (kSB * kSX), 1.f / (kSB * kSX)), sx2 = pk2(kSX, kSX);
+        f2 Da = pk2(0.f, 0.f), Db = Da;
+        uint32_t r[2][16];
+        tmem_ld16(acc_t, r[0]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          tmem_wait_ld();
+          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          uint32_t(&c)[16] = r[q & 1];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) xs[8 * q + j] = fma2(pk2u(c[2 * j], c[2 * j + 1]), k3, mul2(xs[8 * q + j], si2));
+          if (!last) {
+            uint32_t p[4];
+#pragma unroll
+            for (int j = 0; j < 8; j += 2) {
+              Da = fma2(xs[8 * q + j], xs[8 * q + j], Da);
+              Db = fma2(xs[8 * q + j + 1], xs[8 * q + j + 1], Db);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) p[j] = cvt_e4m3x4(mul2(xs[8 * q + 2 * j], sx2), mul2(xs[8 * q + 2 * j + 1], sx2));
+            sts128(chunk_addr(xrow8, q), make_uint4(p[0], p[1], p[2], p[3]));
+            tmem_st4(opa_t + 4 * q, p);
+          }
+        }
+        if (!last) {
+          float d0, d1;
+          upk2(add2(Da, Db), d0, d1);
+          ctrl->dpart[q4][t] = d0 + d1;
+        }
+      }
+      TR();   // E3 loop done
+      if (!last) {
+        ready_and_issue(1);
+        write_xb_copy(xs);
+        di = (ctrl->dpart[0][t] + ctrl->dpart[1][t]) + (ctrl->dpart[2][t] + ctrl->dpart[3][t]);
+      } else {
+        tc_fence_before_sync();
+      }
+      TR();   // MMA1 of the next step issued (or nothing)
+    }
+
+    // ---------------- F: untile + scaled, weight-decayed write --------------------------------
+    if (step_mode) {
+      if (lead && !w_issued) {                               // K = 0: W was not prefetched
+        tma_wait_group_read0();
+        mbar_arrive_expect_tx(w_bar, kBufBytes);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tma_load_2d(ST + j * kBlkBytes, map_w, x0 + 64 * j, y0, w_bar);
+      }
+      mbar_wait(w_bar, ph_w);
+      ph_w ^= 1;
+    } else {
+      if (lead) tma_wait_group_read0();                      // Phi mode: the previous output has left ST
+      __syncthreads();
+    }
+    {
+      const float keep = 1.f - hp.lr * hp.wd;
+      const float unq = 1.f / qs;                                   // undo the c^(1/4) state scaling
+      const float stepsz = step_mode ? -hp.lr * hp.scale_c * tau_base * unq : unq;
+      const f2 step2 = pk2(stepsz, stepsz), keep2 = pk2(keep, keep);
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        uint32_t p[4];
+        if (step_mode) {
+          const uint4 wv = lds128(chunk_addr(srow, c));
+          const uint32_t ww[4] = {wv.x, wv.y, wv.z, wv.w};
+#pragma unroll
+          for (int e = 0; e < 4; ++e)
+            p[e] = cvt_bf16x2(fma2(keep2, pk2u(ww[e] << 16, ww[e] & 0xffff0000u), mul2(step2, xs[4 * c + e])));
+        } else {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) p[e] = cvt_bf16x2(mul2(step2, xs[4 * c + e]));
+        }
+        sts128(chunk_addr(srow, c), make_uint4(p[0], p[1], p[2], p[3]));
+      }
+    }
+    fence_proxy_async_smem();
+    __syncthreads();
+    if (lead) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j) tma_store_2d(map_w, x0 + 64 * j, y0, ST + j * kBlkBytes);
+      tma_commit_group();
+    }
+  }
+
+  if (lead) tma_wait_group0();
+  tc_fence_before_sync();
+  cluster_sync_all();
+  if (warp == 0) tmem_dealloc_pair<512>(tmem_base);
+}
+
+}  // namespace
+
+cudaError_t launch_tc256_fp8(const LaunchArgs& a, cudaStream_t s) {
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(himuon_tc256_fp8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  if (a.n_items < 1) return cudaSuccess;
+  long long clusters = a.n_items;
+  const int max_clusters = device_sm_count() / 2;
+  if (clusters > max_clusters) clusters = max_clusters;
+  himuon_tc256_fp8_kernel<<<(unsigned)(2 * clusters), kThreads, kSmemBytes, s>>>(a.layers, a.tmaps, a.items, a.n_items, a.mode, a.hp);
+  return cudaGetLastError();
+}
+
+}  // namespace himuon

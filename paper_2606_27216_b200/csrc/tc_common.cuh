@@ -39,6 +39,29 @@ __device__ __forceinline__ void pack16(const uint32_t (&r)[16], uint32_t (&p)[8]
   for (int j = 0; j < 8; ++j) p[j] = pack_bf16(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
 }
 
+// ---- e4m3 operands (kernels_tc128_fp8.cu, kernels_tc256_fp8.cu) ----------------------------------
+// four fp32 (two packed pairs) -> four e4m3 bytes, element 0 in the low byte
+__device__ __forceinline__ uint32_t cvt_e4m3x4(f2 v01, f2 v23) {
+  float a, b, c, d;
+  upk2(v01, a, b);
+  upk2(v23, c, d);
+  uint32_t r;
+  asm("{\n\t.reg .b16 lo, hi;\n\tcvt.rn.satfinite.e4m3x2.f32 lo, %2, %1;\n\tcvt.rn.satfinite.e4m3x2.f32 hi, %4, %3;\n\t"
+      "mov.b32 %0, {lo, hi};\n\t}"
+      : "=r"(r) : "f"(a), "f"(b), "f"(c), "f"(d));
+  return r;
+}
+// 16 accumulator columns, scaled by k -> 16 e4m3 (4 words)
+__device__ __forceinline__ void pack16_e4m3(const uint32_t (&r)[16], f2 k2, uint32_t (&p)[4]) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j)
+    p[j] = cvt_e4m3x4(mul2(pk2u(r[4 * j], r[4 * j + 1]), k2), mul2(pk2u(r[4 * j + 2], r[4 * j + 3]), k2));
+}
+// Replace one byte of a packed 16-column chunk: word `idx` (0..3, or 4 for none) becomes (word & keep) | val.
+__device__ __forceinline__ void set_one4(uint32_t (&p)[4], int idx, uint32_t keep, uint32_t val) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j) p[j] = (j == idx) ? ((p[j] & keep) | val) : p[j];
+}
 
 }  // namespace tc
 }  // namespace himuon

@@ -98,14 +98,16 @@ def test_config5_llama3_8b_step(T):
     assert plan.workspace_bytes <= 2048 << 20
 
 
-def test_config5_llama3_8b_step_fp8():
+@pytest.mark.parametrize("T", [128, 256])
+def test_config5_llama3_8b_step_fp8(T):
     """The same full-size launch on the opt-in e4m3-operand path (HIMUON_PATH_FP8), at its own tolerance (0.15)."""
     _need_gpu(120)
-    plan, worst, n = _run_config_step(I.llama3_8b_spec(), 128, 2048, 128, 5, path=hm.HIMUON_PATH_FP8, tol=0.15)
-    assert plan.n_tiles == 425984
+    plan, worst, n = _run_config_step(I.llama3_8b_spec(), T, 2048, 128, 5, path=hm.HIMUON_PATH_FP8, tol=0.15)
+    assert plan.n_tiles == {128: 425984, 256: 106496}[T]
 
 
-def test_config4_gpt2_xl_ragged_fp8_deterministic():
+@pytest.mark.parametrize("T", [128, 256])
+def test_config4_gpt2_xl_ragged_fp8_deterministic(T):
     """GPT-2-XL shapes (64-wide edge tiles) on the e4m3-operand path: two steps from the same bits twice give bitwise
     identical W' and M' (no race between the slots, the prefetches and the stores)."""
     _need_gpu(40)
@@ -117,7 +119,7 @@ def test_config4_gpt2_xl_ragged_fp8_deterministic():
         for i in range(len(spec.layers)):
             W, G, M = I.make_layer_tensors(spec, i, dtype=torch.bfloat16, device=DEV)
             Ws.append(W); Gs.append(G); Ms.append(M)
-        plan = hm.Plan.from_tensors(Ws, Gs, Ms, 128, path=hm.HIMUON_PATH_FP8).bind()
+        plan = hm.Plan.from_tensors(Ws, Gs, Ms, T, path=hm.HIMUON_PATH_FP8).bind()
         plan.step(hp)
         plan.step(hp)
         torch.cuda.synchronize()

@@ -238,15 +238,16 @@ def test_chunk_rule_properties():
     check()
 
 
-def test_fp8_path_is_opt_in_and_T128_only():
-    """HIMUON_PATH_FP8 (e4m3 operands, include/himuon.h): bf16 storage, T = 128, width a multiple of 8 - everything
+def test_fp8_path_is_opt_in_and_T128_T256_only():
+    """HIMUON_PATH_FP8 (e4m3 operands, include/himuon.h): bf16 storage, T = 128 or 256, width a multiple of 8 - everything
     else is refused at plan time, never silently served by another kernel; AUTO never selects it."""
     U = B.HIMUON_ERR_UNSUPPORTED
-    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16, hm.HIMUON_PATH_FP8) == [128]
+    assert hm.himuon_supported_tile_sizes(hm.HIMUON_BF16, hm.HIMUON_PATH_FP8) == [128, 256]
     assert hm.himuon_supported_tile_sizes(hm.HIMUON_F32, hm.HIMUON_PATH_FP8) == []
     p = hm.Plan(_layers([(512, 768), (100, 128)]), 128, path=hm.HIMUON_PATH_FP8)
     assert p.n_tiles == 24 + 1 and p.n_buckets == 1
-    for shapes, T, kw in (([(512, 512)], 64, {}), ([(512, 512)], 256, {}), ([(512, 512)], 512, {}),
+    assert hm.Plan(_layers([(512, 768)]), 256, path=hm.HIMUON_PATH_FP8).n_tiles == 6
+    for shapes, T, kw in (([(512, 512)], 64, {}), ([(512, 500)], 256, {}), ([(512, 512)], 512, {}),
                           ([(512, 500)], 128, {}), ([(512, 512)], 128, {"dtype": hm.HIMUON_F32})):
         with pytest.raises(hm.HimuonError) as e:
             hm.Plan(_layers(shapes, **kw), T, path=hm.HIMUON_PATH_FP8)

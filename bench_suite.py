@@ -47,21 +47,26 @@ def _emit(row):
 def _step_rows(args, hm, pk, dev):
     from bench import spec_of, algorithmic_flops, make_inputs
     hp = hm.HParams(K=args.K, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
-    for name, T, cap in (("gpt2-small", 128, 2048), ("gpt2-xl", 128, 256), ("llama3-8b", 128, 2048),
-                         ("llama3-8b", 64, 2048), ("llama3-8b", 256, 2048), ("llama3-8b-sched", 128, 2048),
-                         ("llama3-8b", 512, 2048), ("llama3-8b", 1 << 20, 2048)):
+    AUTO, FP8 = hm.HIMUON_PATH_AUTO, hm.HIMUON_PATH_FP8
+    for name, T, cap, path in (("gpt2-small", 128, 2048, AUTO), ("gpt2-xl", 128, 256, AUTO), ("llama3-8b", 128, 2048, AUTO),
+                               ("llama3-8b", 64, 2048, AUTO), ("llama3-8b", 256, 2048, AUTO), ("llama3-8b-sched", 128, 2048, AUTO),
+                               ("llama3-8b", 512, 2048, AUTO), ("llama3-8b", 1 << 20, 2048, AUTO),
+                               ("llama3-8b", 128, 2048, FP8), ("llama3-8b", 256, 2048, FP8)):   # opt-in e4m3 operands
         spec = spec_of(name)
         row = {"row": "step", "workload": name, "T": T, "cap_mb": cap}
+        if path == FP8:
+            row["path"] = "fp8 (e4m3 operands; reduced precision; peak = bf16 peak x 2)"
         try:
             n_sets = max(1, -(-2 * L2_BYTES // (10 * spec.n_elements)))     # rotate copies until > 2 x L2
             sets = [make_inputs(spec, dev) for _ in range(n_sets)]
             Tl = [l.T for l in spec.layers]
-            plans = [hm.Plan.from_tensors(W, G, M, T, T_per_layer=Tl if any(Tl) else None,
+            plans = [hm.Plan.from_tensors(W, G, M, T, T_per_layer=Tl if any(Tl) else None, path=path,
                                           workspace_cap_bytes=cap << 20).bind() for (W, G, M) in sets]
             flops = algorithmic_flops(spec, T, args.K) if T <= 512 else float(sum(
                 6.0 * args.K * min(l.H, l.W) * l.H * l.W for l in spec.layers))   # full matrix: Gram on the short side
             med, best = _time(lambda i: plans[i % n_sets].step(hp), args.steps if T <= 256 else 2)
-            bound, roof_ms = _roof(flops, 10.0 * spec.n_elements, pk)
+            bound, roof_ms = _roof(flops, 10.0 * spec.n_elements,
+                                   dict(pk, bf16_sustained=2 * pk["bf16_sustained"]) if path == FP8 else pk)
             row.update({"ms": round(med, 4), "ms_min": round(best, 4), "tflops": round(flops / med / 1e9, 2),
                         "gbs": round(10.0 * spec.n_elements / med / 1e6, 1), "bound": bound,
                         "roofline_ms": round(roof_ms, 4), "frac": round(roof_ms / med, 4), "tiles": plans[0].n_tiles,

@@ -159,3 +159,39 @@ def test_fp8_capacity_diagnostic(T):
           f"to the same-input oracle {gap_b:.3e}")
     assert abs(n_got - n_ref) <= 15
     assert gap_b <= TOL_FP8
+
+
+@pytest.mark.parametrize("T,N", [(128, 37), (256, 9)])
+def test_fp8_ns_tiles_packed_batch(T, N):
+    """himuon_ns_tiles on a packed [N, T, T] batch (the Fig. 7 workload) through the fp8 path."""
+    _need_gpu()
+    tiles = I.row_scaled_gaussian(N * T, T, seed_cfg=50, dtype=torch.bfloat16).reshape(N, T, T).contiguous()
+    out = hm.himuon_ns_tiles(tiles.to(DEV), K=5, eps=1e-7, path=hm.HIMUON_PATH_FP8)
+    torch.cuda.synchronize()
+    got = PU.f64(out.cpu())
+    worst = 0.0
+    for i in range(N):
+        ref = PU.O.phi(PU.f64(tiles[i]), 5, eps=float(np.float32(1e-7)))
+        worst = max(worst, float(np.linalg.norm(got[i] - ref) / np.linalg.norm(ref)))
+    assert np.all(np.isfinite(got)) and worst <= TOL_FP8, f"worst tile error {worst:.3e}"
+
+
+@pytest.mark.parametrize("T", [128, 256])
+def test_fp8_chunked_equals_unchunked(T):
+    """The workspace cap splits the work list into chunks; chunking must not change a bit."""
+    _need_gpu()
+    G = _inputs(4 * T, 6 * T, 51)
+    hp = hm.HParams(K=5, eps=1e-7)
+    probe = hm.Plan.from_tensors([torch.empty_like(G)], [G], None, T, path=hm.HIMUON_PATH_FP8)
+    fixed = probe.workspace_bytes - 16 * probe.n_tiles
+    outs = []
+    for cap in (0, fixed + 16 * 5):
+        Gd = G.to(DEV)
+        Ud = torch.full_like(Gd, float("nan"))
+        plan = hm.Plan.from_tensors([Ud], [Gd], None, T, path=hm.HIMUON_PATH_FP8, workspace_cap_bytes=cap).bind()
+        plan.phi(hp)
+        torch.cuda.synchronize()
+        outs.append((Ud.cpu(), plan.n_chunks))
+        plan.destroy()
+    assert outs[0][1] == 1 and outs[1][1] >= 3
+    assert torch.equal(outs[0][0], outs[1][0])

@@ -143,7 +143,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   const float beta_h = hp.b / sqrtf(hp.c);
 
   // Operands of the next pair MMA are written: tell the leader; the leader issues once both CTAs have.
-  // which: 1 = MMA1 (B = XB, K-major), 2 = MMA2 (B = OB, K-major), 3 = MMA3 (B = Xb copy in ST, MN-major).
+  // which: 1 = MMA1 (B = Xb in OB, K-major), 2 = MMA2 (B = Ot in XB, K-major), 3 = MMA3 (B = Xb copy in ST, MN-major).
   auto ready_and_issue = [&](int which) {
     tmem_wait_st();
     // generic-proxy writes -> visible to the MMA.  Remote (DSMEM) writes happen only in write_xb_copy, between the
@@ -158,7 +158,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       if (rank == 0) {
         mbar_wait_cluster(ready_bar, ph_ready);
         tc_fence_after_sync();
-        issue_pair(ACCd, OPAd, which == 1 ? XB : which == 2 ? OB : ST, which == 3, mma_bar);
+        issue_pair(ACCd, OPAd, which == 1 ? OB : which == 2 ? XB : ST, which == 3, mma_bar);
       }
     }
     ph_ready ^= 1;
@@ -221,12 +221,12 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     // ---------------- P: load, momentum, normalise ---------------------------------------------------
     if (lead) {
       if (!prefetched) issue_gm(it);
-      tma_wait_group_read0();   // the previous tile's stores out of ST have been read: M' may be written into it
       mbar_arrive(ld_bar);
     }
     mbar_wait(ld_bar, ph_ld);
     ph_ld ^= 1;
     prefetched = false;
+    TR();   // G, M landed and the staging buffer is free
 
     f2 xs[32];                  // fp32 state: this thread's 64 columns of row R, as packed pairs
     f2 ss2 = pk2(0.f, 0.f);
@@ -248,7 +248,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           ss2 = fma2(h2, h2, ss2);
           xs[4 * c + e] = h2;
         }
-        sts128(chunk_addr(srow, c), make_uint4(mo[0], mo[1], mo[2], mo[3]));
+        sts128(chunk_addr(xrow, c), make_uint4(mo[0], mo[1], mo[2], mo[3]));   // M' in place, over this thread's M
       } else {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
@@ -265,21 +265,31 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
     if (lane == 0) ctrl->red[warp] = tot;
-    fence_proxy_async_smem();          // M' in ST -> visible to the TMA store
+    fence_proxy_async_smem();          // M' in XB -> visible to the TMA store
     __syncthreads();
+    TR();   // momentum pass done
     float mine = 0.f;
 #pragma unroll
     for (int i = 0; i < 16; ++i) mine += ctrl->red[i];
     if (lead) {
+      // M' leaves from XB, where it was computed in place: nothing waits for that store here (XB is next written
+      // by E1 of the first step, thousands of cycles later).  What must have drained before the cluster barrier
+      // below is the PREVIOUS tile's store out of ST: after the barrier ST of BOTH CTAs may receive the Xb copy.
+      // (A TMA store of 64 KB takes ~3000 cycles to drain at this SM's share of the HBM write bandwidth.  Writing
+      // W' to global memory straight from the registers instead, with no store pending on ST, was measured too:
+      // 66.0 ms against 62.2 ms - the LSU store path costs more than the drain.)
       if (step_mode) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) tma_store_2d(map_m, x0 + 64 * j, y0, ST + j * kBlkBytes);
+        for (int j = 0; j < 4; ++j) tma_store_2d(map_m, x0 + 64 * j, y0, XB + j * kBlkBytes);
         tma_commit_group();
-        tma_wait_group_read0();   // after the cluster barrier below, ST of BOTH CTAs may receive the Xb copy
+        tma_wait_group_read1();
+      } else {
+        tma_wait_group_read0();
       }
       st_cluster_f32(mapa_shared(smem_u32(&ctrl->peer_ss), rank ^ 1u), mine);   // Frobenius norm spans both CTAs
     }
     cluster_sync_all();
+    TR();   // M' on its way, norm exchanged
     tot = mine + ctrl->peer_ss;
     const float nrm = sqrtf(tot);
     const float inv = nrm > 0.f ? qs / (nrm + hp.eps) : 0.f;   // Phi_K(0) = 0
@@ -294,8 +304,8 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           xs[8 * q + j] = mul2(xs[8 * q + j], inv2);
           p[j] = cvt_bf16x2(xs[8 * q + j]);
         }
-        sts128(chunk_addr(xrow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
-        sts128(chunk_addr(xrow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
+        sts128(chunk_addr(orow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));    // Xb lives in OB (G is consumed),
+        sts128(chunk_addr(orow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));  // Ot in XB: see the M' store above
         tmem_st8(opa_t + 8 * q, p);
       }
     }
@@ -311,6 +321,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     for (int k = 0; k < hp.K; ++k) {
       const bool last = (k + 1 == hp.K);
       // ---- E1: ACC = rows of Ah
+      if (lead && k == 0 && step_mode) tma_wait_group_read0();   // M' has left XB (long ago): Ot may be written into it
       wait_mma();
       TR();   // MMA1 done
       {
@@ -333,8 +344,8 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           uint32_t p[8];
           pack16(c, p);
           if (own) set_one(p, dq == q ? dword : 8, dkeep, dval);
-          sts128(chunk_addr(orow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
-          sts128(chunk_addr(orow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
+          sts128(chunk_addr(xrow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
+          sts128(chunk_addr(xrow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
           tmem_st8(opa_t + 8 * q, p);
         }
         float s0, s1;
@@ -401,8 +412,8 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
             }
 #pragma unroll
             for (int j = 0; j < 8; ++j) p[j] = cvt_bf16x2(xs[8 * q + j]);
-            sts128(chunk_addr(xrow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
-            sts128(chunk_addr(xrow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
+            sts128(chunk_addr(orow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
+            sts128(chunk_addr(orow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
             tmem_st8(opa_t + 8 * q, p);
           }
         }
@@ -437,6 +448,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       if (lead) tma_wait_group_read0();                      // Phi mode: the previous output has left ST
       __syncthreads();
     }
+    TR();   // W landed
     {
       const float keep = 1.f - hp.lr * hp.wd;
       const float unq = 1.f / qs;                                   // undo the c^(1/4) state scaling

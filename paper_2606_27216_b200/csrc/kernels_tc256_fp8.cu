@@ -142,7 +142,7 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
       if (rank == 0) {
         mbar_wait_cluster(ready_bar, ph_ready);
         tc_fence_after_sync();
-        issue_pair(ACCd, OPAd, which == 1 ? XB : which == 2 ? OB : ST, which == 3, mma_bar);
+        issue_pair(ACCd, OPAd, which == 1 ? OB : which == 2 ? XB : ST, which == 3, mma_bar);
       }
     }
     ph_ready ^= 1;
@@ -198,7 +198,6 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
     // ---------------- P: load, momentum, normalise ---------------------------------------------------
     if (lead) {
       if (!prefetched) issue_gm(it);
-      tma_wait_group_read0();   // the previous tile's stores out of ST have been read: M' may be written into it
       mbar_arrive(ld_bar);
     }
     mbar_wait(ld_bar, ph_ld);
@@ -225,7 +224,7 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
           ss2 = fma2(h2, h2, ss2);
           xs[4 * c + e] = h2;
         }
-        sts128(chunk_addr(srow, c), make_uint4(mo[0], mo[1], mo[2], mo[3]));
+        sts128(chunk_addr(xrow, c), make_uint4(mo[0], mo[1], mo[2], mo[3]));   // M' in place, over this thread's M
       } else {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
@@ -242,17 +241,22 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
     if (lane == 0) ctrl->red[warp] = tot;
-    fence_proxy_async_smem();          // M' in ST -> visible to the TMA store
+    fence_proxy_async_smem();          // M' in XB -> visible to the TMA store
     __syncthreads();
     float mine = 0.f;
 #pragma unroll
     for (int i = 0; i < 16; ++i) mine += ctrl->red[i];
     if (lead) {
+      // As in kernels_tc256.cu: M' is stored from XB, where it was computed in place, and nothing waits for that
+      // store here; only the PREVIOUS tile's store out of ST must have drained before the cluster barrier below,
+      // after which ST of both CTAs may receive the Xb copy.  Xb lives in OB, Ot in XB.
       if (step_mode) {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) tma_store_2d(map_m, x0 + 64 * j, y0, ST + j * kBlkBytes);
+        for (int j = 0; j < 4; ++j) tma_store_2d(map_m, x0 + 64 * j, y0, XB + j * kBlkBytes);
         tma_commit_group();
-        tma_wait_group_read0();   // after the cluster barrier below, ST of BOTH CTAs may receive the Xb copy
+        tma_wait_group_read1();
+      } else {
+        tma_wait_group_read0();
       }
       st_cluster_f32(mapa_shared(smem_u32(&ctrl->peer_ss), rank ^ 1u), mine);   // Frobenius norm spans both CTAs
     }
@@ -270,7 +274,7 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
         for (int j = 0; j < 8; ++j) xs[8 * q + j] = mul2(xs[8 * q + j], inv2);
 #pragma unroll
         for (int j = 0; j < 4; ++j) p[j] = cvt_e4m3x4(mul2(xs[8 * q + 2 * j], sx2), mul2(xs[8 * q + 2 * j + 1], sx2));
-        sts128(chunk_addr(xrow8, q), make_uint4(p[0], p[1], p[2], p[3]));
+        sts128(chunk_addr(orow8, q), make_uint4(p[0], p[1], p[2], p[3]));
         tmem_st4(opa_t + 4 * q, p);
       }
     }
@@ -286,6 +290,7 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
     for (int k = 0; k < hp.K; ++k) {
       const bool last = (k + 1 == hp.K);
       // ---- E1: ACC = rows of Ah
+      if (lead && k == 0 && step_mode) tma_wait_group_read0();   // M' has left XB (long ago): Ot may be written into it
       wait_mma();
       TR();   // MMA1 done
       {
@@ -310,7 +315,7 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
           uint32_t p[4];
           pack16_e4m3(c, k1, p);
           if (own) set_one4(p, dq == q ? dword : 4, dkeep, dval);
-          sts128(chunk_addr(orow8, q), make_uint4(p[0], p[1], p[2], p[3]));
+          sts128(chunk_addr(xrow8, q), make_uint4(p[0], p[1], p[2], p[3]));
           tmem_st4(opa_t + 4 * q, p);
         }
         float s0, s1;
@@ -378,7 +383,7 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
             }
 #pragma unroll
             for (int j = 0; j < 4; ++j) p[j] = cvt_e4m3x4(mul2(xs[8 * q + 2 * j], sx2), mul2(xs[8 * q + 2 * j + 1], sx2));
-            sts128(chunk_addr(xrow8, q), make_uint4(p[0], p[1], p[2], p[3]));
+            sts128(chunk_addr(orow8, q), make_uint4(p[0], p[1], p[2], p[3]));
             tmem_st4(opa_t + 4 * q, p);
           }
         }

@@ -352,15 +352,15 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
       // ---- E3: Xh = (a + B_RR) Xh + offdiag(B) Xh
       wait_mma();
       TR();   // MMA3 done
-      if (last && nxt < n_items) {                           // XB and OB are free (every pair MMA has completed)
-        if (lead) issue_gm(nxt);
-        prefetched = true;
-      }
-      if (last && lead && step_mode) {                       // ... and so is ST: fetch W into it
-        mbar_arrive_expect_tx(w_bar, kBufBytes);
+      if (last && lead && step_mode) {                       // ST is free (every pair MMA has completed): fetch W into
+        mbar_arrive_expect_tx(w_bar, kBufBytes);             // it - FIRST, phase F needs it long before P needs G, M
 #pragma unroll
         for (int j = 0; j < 4; ++j) tma_load_2d(ST + j * kBlkBytes, map_w, x0 + 64 * j, y0, w_bar);
         w_issued = true;
+      }
+      if (last && nxt < n_items) {                           // ... and so are XB and OB: the next tile's G and M
+        if (lead) issue_gm(nxt);
+        prefetched = true;
       }
       {
         const f2 si2 = pk2(si, si), k3 = pk2(1.f / (kSB * kSX), 1.f / (kSB * kSX)), sx2 = pk2(kSX, kSX);

@@ -2,8 +2,10 @@
 
     python -m paper_2606_27216_b200.build [--force] [--verbose]
 
-nvcc cross-compiles without a GPU.  The shared object lands next to this file so that it travels
-with the repository snapshot to the GPU box (it is git-ignored).
+nvcc cross-compiles without a GPU.  Every .cu is compiled to its own object (in parallel, cached by a
+fingerprint of the source, the headers and the flags) and the objects are linked into the shared object,
+which lands next to this file so that it travels with the repository snapshot to the GPU box (it is
+git-ignored).
 """
 from __future__ import annotations
 
@@ -11,22 +13,25 @@ import hashlib
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG_DIR)
 CSRC = os.path.join(PKG_DIR, "csrc")
+OBJ_DIR = os.path.join(PKG_DIR, "build")
 LIB_PATH = os.path.join(PKG_DIR, "libhimuon.so")
 STAMP_PATH = os.path.join(PKG_DIR, "libhimuon.stamp")
 
-SOURCES = ["himuon_api.cu", "kernels_simt.cu", "kernels_tc128.cu", "kernels_tc128_fp8.cu", "kernels_tc64.cu", "kernels_tc256.cu", "kernels_tc256_fp8.cu", "kernels_warp.cu", "kernels_gemm.cu"]
-HEADERS = ["himuon_internal.h", "sm100_ptx.cuh", "tc_common.cuh", os.path.join(ROOT, "include", "himuon.h")]
+SOURCES = sorted(f for f in os.listdir(CSRC) if f.endswith(".cu"))
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))) + [os.path.join(ROOT, "include", "himuon.h")]
 
-NVCC_FLAGS = [
+COMPILE_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared", "-ldl",
+    "-Xcompiler", "-fPIC",
     "-I", os.path.join(ROOT, "include"), "-I", CSRC,
 ]
+LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC", "-ldl"]
 
 
 def _nvcc() -> str:
@@ -36,33 +41,73 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def _fingerprint() -> str:
+def _read(path: str) -> bytes:
+    with open(path, "rb") as fh:
+        return fh.read()
+
+
+def _header_hash() -> str:
     h = hashlib.sha256()
-    for f in SOURCES + HEADERS:
-        p = f if os.path.isabs(f) else os.path.join(CSRC, f)
-        with open(p, "rb") as fh:
-            h.update(fh.read())
-    h.update(" ".join(NVCC_FLAGS).encode())
+    for f in HEADERS:
+        h.update(_read(f if os.path.isabs(f) else os.path.join(CSRC, f)))
     return h.hexdigest()
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile if sources changed; return the path of the shared library."""
-    fp = _fingerprint()
-    if not force and os.path.exists(LIB_PATH) and os.path.exists(STAMP_PATH):
-        with open(STAMP_PATH) as fh:
-            if fh.read().strip() == fp:
-                return LIB_PATH
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB_PATH]
+def _fingerprint(extra_flags=()) -> str:
+    h = hashlib.sha256()
+    for f in SOURCES:
+        h.update(_read(os.path.join(CSRC, f)))
+    h.update(_header_hash().encode())
+    h.update(" ".join(COMPILE_FLAGS + LINK_FLAGS + list(extra_flags)).encode())
+    return h.hexdigest()
+
+
+def _compile_one(src: str, obj_dir: str, hdr: str, extra_flags, force: bool, verbose: bool):
+    """Compile csrc/<src> -> <obj_dir>/<src>.o unless its fingerprint is unchanged; returns (obj, log)."""
+    obj = os.path.join(obj_dir, src + ".o")
+    stamp = obj + ".stamp"
+    h = hashlib.sha256(_read(os.path.join(CSRC, src)))
+    h.update(hdr.encode())
+    h.update(" ".join(COMPILE_FLAGS + list(extra_flags)).encode())
+    fp = h.hexdigest()
+    if not force and os.path.exists(obj) and os.path.exists(stamp) and _read(stamp).decode().strip() == fp:
+        return obj, ""
+    cmd = [_nvcc()] + COMPILE_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + \
+          ["-c", os.path.join(CSRC, src), "-o", obj]
     res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libhimuon.so (see stderr)")
-    with open(STAMP_PATH, "w") as fh:
+        raise RuntimeError(f"nvcc failed on {src}:\n{res.stdout}{res.stderr}")
+    with open(stamp, "w") as fh:
         fh.write(fp)
-    return LIB_PATH
+    return obj, res.stdout + res.stderr
+
+
+def build(force: bool = False, verbose: bool = False, extra_flags=(), lib_path: str = LIB_PATH,
+          obj_dir: str = OBJ_DIR) -> str:
+    """Compile what changed, link, and return the path of the shared library.
+
+    `extra_flags` / `lib_path` / `obj_dir` let a development build (e.g. -DHIMUON_TRACE) live beside the product
+    library without touching it."""
+    stamp_path = STAMP_PATH if lib_path == LIB_PATH else lib_path + ".stamp"
+    fp = _fingerprint(extra_flags)
+    if not force and os.path.exists(lib_path) and os.path.exists(stamp_path):
+        if _read(stamp_path).decode().strip() == fp:
+            return lib_path
+    os.makedirs(obj_dir, exist_ok=True)
+    hdr = _header_hash()
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as pool:
+        results = list(pool.map(lambda s: _compile_one(s, obj_dir, hdr, extra_flags, force, verbose), SOURCES))
+    if verbose:
+        for _, log in results:
+            sys.stderr.write(log)
+    cmd = [_nvcc()] + LINK_FLAGS + [o for o, _ in results] + ["-o", lib_path]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed linking libhimuon.so (see stderr)")
+    with open(stamp_path, "w") as fh:
+        fh.write(fp)
+    return lib_path
 
 
 if __name__ == "__main__":

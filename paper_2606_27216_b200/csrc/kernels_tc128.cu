@@ -45,6 +45,14 @@ namespace himuon {
 
 int g_tc128_debug_stage = 0;   // 0 = normal; 1/2 = dump ACC after MMA1 / MMA2 of the first step (tests only)
 
+#ifdef HIMUON_TRACE   // development aid (not built into libhimuon.so): clock stamps of the two lead threads of CTA 0
+__device__ long long g_trace128[2][16384];
+__device__ int g_tn128[2];
+#define TR(id) do { if (lead && blockIdx.x == 0 && g_tn128[slot] < 16384) g_trace128[slot][g_tn128[slot]++] = ((long long)(id) << 48) | (clock64() & 0xffffffffffffLL); } while (0)
+#else
+#define TR(id) do { } while (0)
+#endif
+
 namespace {
 
 using namespace ptx;
@@ -115,9 +123,12 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   Ctrl* ctrl = reinterpret_cast<Ctrl*>(smem_raw + (smem0 - smem_u32(smem_raw)) + kSlots * kSlotBytes);
 
   const int tid = threadIdx.x;
-  const int slot = tid / kSlotThreads;
+  // warp-uniform in the compiler's eyes too (a shuffle result is uniform): everything the MMA issue derives from
+  // it - descriptors, TMEM addresses, barrier addresses - then lives in uniform registers
+  const int warp_id = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int slot = warp_id / (kSlotThreads / 32);
   const int ts = tid % kSlotThreads;
-  const int w = ts >> 5;               // warp of the slot
+  const int w = warp_id % (kSlotThreads / 32);   // warp of the slot
   const int wq = w & 3;                // TMEM lane quadrant of this warp (= warp index in the CTA mod 4)
   const int h = w >> 2;                // column half
   const int lane = tid & 31;
@@ -207,12 +218,14 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     const uint32_t dkeep = (t & 1) ? 0x0000ffffu : 0xffff0000u;
 
     // ---------------- P: momentum, normalise ---------------------------------------------------
+    TR(0);
     if (lead) {
       tma_wait_group_read0();   // the previous tile's stores out of ST have been read
       mbar_arrive(ld_bar);
     }
     mbar_wait(ld_bar, ph_ld);
     ph_ld ^= 1;
+    TR(1);
 
     f2 xs[32];                  // fp32 state: this thread's 64 columns of row t, as packed pairs
     float ss = 0.f;             // sum of squares of this thread's part of Ghat
@@ -252,6 +265,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     if (lane == 0) sc->red[w] = tot;
     fence_proxy_async_smem();          // M' in ST -> visible to the TMA store
     named_bar_sync(bar_id, kSlotThreads);
+    TR(2);
     if (lead && step_mode) {
       tma_store_2d(map_m, x0, y0, ST);
       tma_store_2d(map_m, x0 + 64, y0, ST + kHalfBytes);
@@ -282,10 +296,15 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     fence_proxy_async_smem();
     tc_fence_before_sync();
     named_bar_sync(bar_id, kSlotThreads);
-    if (lead && hp.K > 0) {
-      tc_fence_after_sync();
-      issue_gram(ACCd, OPAd, XB, 0u, mma_bar);
+    TR(3);
+    if (w == 0 && hp.K > 0) {
+      if (elect_one()) {
+        tc_fence_after_sync();
+        issue_gram(ACCd, OPAd, XB, 0u, mma_bar);
+      }
+      __syncwarp();
     }
+    TR(4);
     float di = sc->dpart[0][t] + sc->dpart[1][t];   // d_t = (Ah)_tt in fp32, from the fp32 state
 
     bool dumped = false;   // debug stages: xs holds a raw accumulator dump instead of X_K
@@ -297,6 +316,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       wait_mma();
       ph_mma ^= 1;
       tc_fence_after_sync();
+      TR(10);
       if (dbg == 1) { dumped = true; break; }
       {
         // Ot = offdiag(Ah) + diag(d + beta/2), rounded to bf16: then for i != j
@@ -338,11 +358,17 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       tmem_wait_st();
       fence_proxy_async_smem();
       tc_fence_before_sync();
+      TR(11);
       named_bar_sync(bar_id, kSlotThreads);
-      if (lead) {
-        tc_fence_after_sync();
-        issue_gram(ACCd, OPAd, OB, 0u, mma_bar);
+      TR(12);
+      if (w == 0) {
+        if (elect_one()) {
+          tc_fence_after_sync();
+          issue_gram(ACCd, OPAd, OB, 0u, mma_bar);
+        }
+        __syncwarp();
       }
+      TR(13);
       // a + B_tt, B_tt = beta d_t + (Ah^2)_tt
       const float si = hp.a + fmaf(beta_h, di, sc->spart[0][t] + sc->spart[1][t]);
 
@@ -350,6 +376,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       wait_mma();
       ph_mma ^= 1;
       tc_fence_after_sync();
+      TR(20);
       if (dbg == 2) { dumped = true; break; }
       if (lead && last && nxt < n_items) {                  // OB is free: fetch the next tile's G
         issue_g(nxt);
@@ -371,16 +398,23 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       }
       tmem_wait_st();
       tc_fence_before_sync();
+      TR(21);
       named_bar_sync(bar_id, kSlotThreads);
-      if (lead) {
-        tc_fence_after_sync();
-        issue_bx(ACCd, OPAd, XB, mma_bar);
+      TR(22);
+      if (w == 0) {
+        if (elect_one()) {
+          tc_fence_after_sync();
+          issue_bx(ACCd, OPAd, XB, mma_bar);
+        }
+        __syncwarp();
       }
+      TR(23);
 
       // ---- E3: Xh = (a + B_tt) Xh + offdiag(B) Xh
       wait_mma();
       ph_mma ^= 1;
       tc_fence_after_sync();
+      TR(30);
       if (lead && last && step_mode && g_issued) {          // XB is free: fetch the next tile's M
         issue_m(nxt);
         m_issued = true;
@@ -421,11 +455,17 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         tmem_wait_st();
         fence_proxy_async_smem();
         tc_fence_before_sync();
+        TR(31);
         named_bar_sync(bar_id, kSlotThreads);
-        if (lead) {
-          tc_fence_after_sync();
-          issue_gram(ACCd, OPAd, XB, 0u, mma_bar);
+        TR(32);
+        if (w == 0) {
+          if (elect_one()) {
+            tc_fence_after_sync();
+            issue_gram(ACCd, OPAd, XB, 0u, mma_bar);
+          }
+          __syncwarp();
         }
+        TR(33);
         di = sc->dpart[0][t] + sc->dpart[1][t];
       }
     }
@@ -442,6 +482,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     }
 
     // ---------------- F: untile + scaled, weight-decayed write --------------------------------
+    TR(40);
     if (step_mode) {
       if (lead && !w_issued) {                               // K = 0 or a debug stage: W was not prefetched
         tma_wait_group_read0();
@@ -452,6 +493,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       mbar_wait(w_bar, ph_w);
       ph_w ^= 1;
     }
+    TR(41);
     {
       const float keep = 1.f - hp.lr * hp.wd;
       const float unq = dbg ? 1.f : 1.f / qs;                       // undo the c^(1/4) state scaling
@@ -474,7 +516,9 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       }
     }
     fence_proxy_async_smem();
+    TR(42);
     named_bar_sync(bar_id, kSlotThreads);
+    TR(43);
     if (lead) {
       tma_store_2d(map_w, x0, y0, ST);
       tma_store_2d(map_w, x0 + 64, y0, ST + kHalfBytes);
@@ -484,6 +528,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         if (step_mode && !m_issued) issue_m(nxt);
       }
     }
+    TR(44);
   }
 
   if (lead) tma_wait_group0();
@@ -513,3 +558,13 @@ cudaError_t launch_tc128(const LaunchArgs& a, cudaStream_t s) {
 }  // namespace himuon
 
 extern "C" void himuon_debug_set_tc128_stage(int stage) { himuon::g_tc128_debug_stage = stage; }
+#ifdef HIMUON_TRACE
+extern "C" int himuon_debug_read_trace128(long long* out, int* n) {
+  cudaMemcpyFromSymbol(n, himuon::g_tn128, sizeof(int) * 2, 0, cudaMemcpyDeviceToHost);
+  return (int)cudaMemcpyFromSymbol(out, himuon::g_trace128, sizeof(long long) * 2 * 16384, 0, cudaMemcpyDeviceToHost);
+}
+extern "C" int himuon_debug_reset_trace128() {
+  int z[2] = {0, 0};
+  return (int)cudaMemcpyToSymbol(himuon::g_tn128, z, sizeof(z));
+}
+#endif

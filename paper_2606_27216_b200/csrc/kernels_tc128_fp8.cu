@@ -101,9 +101,12 @@ himuon_tc128_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
   Ctrl* ctrl = reinterpret_cast<Ctrl*>(smem_raw + (smem0 - smem_u32(smem_raw)) + kSlots * kSlotBytes);
 
   const int tid = threadIdx.x;
-  const int slot = tid / kSlotThreads;
+  // warp-uniform in the compiler's eyes too (a shuffle result is uniform): what the MMA issue derives from it
+  // (descriptors, TMEM and barrier addresses) then lives in uniform registers
+  const int warp_id = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int slot = warp_id / (kSlotThreads / 32);
   const int ts = tid % kSlotThreads;
-  const int w = ts >> 5;               // warp of the slot
+  const int w = warp_id % (kSlotThreads / 32);   // warp of the slot
   const int wq = w & 3;                // TMEM lane quadrant of this warp (= warp index in the CTA mod 4)
   const int h = w >> 2;                // column half
   const int lane = tid & 31;
@@ -270,9 +273,12 @@ himuon_tc128_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
     fence_proxy_async_smem();
     tc_fence_before_sync();
     named_bar_sync(bar_id, kSlotThreads);
-    if (lead && hp.K > 0) {
-      tc_fence_after_sync();
-      issue_gram(ACCd, OPAd, XB, mma_bar);
+    if (w == 0 && hp.K > 0) {
+      if (elect_one()) {
+        tc_fence_after_sync();
+        issue_gram(ACCd, OPAd, XB, mma_bar);
+      }
+      __syncwarp();
     }
     float di = sc->dpart[0][t] + sc->dpart[1][t];   // d_t = (Ah)_tt in fp32, from the fp32 state
 
@@ -329,9 +335,12 @@ himuon_tc128_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
       fence_proxy_async_smem();
       tc_fence_before_sync();
       named_bar_sync(bar_id, kSlotThreads);
-      if (lead) {
-        tc_fence_after_sync();
-        issue_gram(ACCd, OPAd, OB, mma_bar);
+      if (w == 0) {
+        if (elect_one()) {
+          tc_fence_after_sync();
+          issue_gram(ACCd, OPAd, OB, mma_bar);
+        }
+        __syncwarp();
       }
       // a + B_tt, B_tt = beta d_t + (Ah^2)_tt
       const float si = hp.a + fmaf(beta_h, di, sc->spart[0][t] + sc->spart[1][t]);
@@ -362,9 +371,12 @@ himuon_tc128_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
       tmem_wait_st();
       tc_fence_before_sync();
       named_bar_sync(bar_id, kSlotThreads);
-      if (lead) {
-        tc_fence_after_sync();
-        issue_bx(ACCd, OPAd, XB, mma_bar);
+      if (w == 0) {
+        if (elect_one()) {
+          tc_fence_after_sync();
+          issue_bx(ACCd, OPAd, XB, mma_bar);
+        }
+        __syncwarp();
       }
 
       // ---- E3: Xh = (a + B_tt) Xh + offdiag(B) Xh
@@ -411,9 +423,12 @@ himuon_tc128_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
         fence_proxy_async_smem();
         tc_fence_before_sync();
         named_bar_sync(bar_id, kSlotThreads);
-        if (lead) {
-          tc_fence_after_sync();
-          issue_gram(ACCd, OPAd, XB, mma_bar);
+        if (w == 0) {
+          if (elect_one()) {
+            tc_fence_after_sync();
+            issue_gram(ACCd, OPAd, XB, mma_bar);
+          }
+          __syncwarp();
         }
         di = sc->dpart[0][t] + sc->dpart[1][t];
       }

@@ -92,7 +92,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   Ctrl* ctrl = reinterpret_cast<Ctrl*>(smem_raw + (smem0 - smem_u32(smem_raw)) + 3 * kBufBytes);
 
   const int tid = threadIdx.x;
-  const int warp = tid >> 5;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // warp-uniform for the compiler too: the MMA issue stays in uniform registers
   const int wq = warp & 3;             // TMEM lane quadrant of this warp
   const int q4 = warp >> 2;            // column quarter
   const int lane = tid & 31;
@@ -153,13 +153,16 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     else if (which == 1) fence_proxy_async_smem();
     tc_fence_before_sync();
     __syncthreads();
-    if (lead) {
-      mbar_arrive_cluster(ready_bar_leader);
-      if (rank == 0) {
-        mbar_wait_cluster(ready_bar, ph_ready);
-        tc_fence_after_sync();
-        issue_pair(ACCd, OPAd, which == 1 ? OB : which == 2 ? XB : ST, which == 3, mma_bar);
+    if (warp == 0) {
+      if (elect_one()) {
+        mbar_arrive_cluster(ready_bar_leader);
+        if (rank == 0) {
+          mbar_wait_cluster(ready_bar, ph_ready);
+          tc_fence_after_sync();
+          issue_pair(ACCd, OPAd, which == 1 ? OB : which == 2 ? XB : ST, which == 3, mma_bar);
+        }
       }
+      __syncwarp();
     }
     ph_ready ^= 1;
   };

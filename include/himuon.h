@@ -24,8 +24,12 @@
  *   - Errors are return codes; nothing throws across this boundary.  Argument validation happens
  *     before any launch.  There is NO CPU fallback: on a machine without a usable sm_100 device the
  *     compute entry points return HIMUON_ERR_CUDA.
- *   - The plan is immutable and holds no optimizer state: momentum lives in the caller's M
- *     buffers and survives re-planning with a different T.
+ *   - The plan's work list, buckets and chunks are fixed at himuon_plan_create; the only thing that changes
+ *     afterwards is which workspace it is bound to (himuon_plan_bind).  It holds no optimizer state: momentum
+ *     lives in the caller's M buffers and survives re-planning with a different T.
+ *   - Thread safety: distinct plans may be created, bound and stepped from different host threads and on
+ *     different devices concurrently (kernel configuration is per device); one plan is used by one thread
+ *     at a time.
  */
 #ifndef HIMUON_H_
 #define HIMUON_H_
@@ -67,7 +71,10 @@ typedef enum { HIMUON_F32 = 0, HIMUON_BF16 = 1 } himuon_dtype;
  *          iterate, the diagonals of A and B, momentum and update stay fp32.  Opt-in:
  *          per-tile error about 0.1 instead of <= 3e-2 on Gaussian-like and low-rank tiles, and a heavy-tailed
  *          tile dominated by a few entries (Student-t with 2 degrees of freedom) can leave the basin of the quintic:
- *          the result is then finite but wrong by O(1) or more.  Never selected by AUTO. */
+ *          the result is then finite but wrong by O(1) or more.  Never selected by AUTO.
+ *          Edge tiles with fewer than 32 live rows or columns are run by the bf16 kernel of the same tile size (their
+ *          own bucket of the plan, visible through himuon_plan_worklist): too few singular directions to average
+ *          e4m3 roundings over. */
 typedef enum { HIMUON_PATH_AUTO = 0, HIMUON_PATH_FP32 = 1, HIMUON_PATH_FP8 = 2 } himuon_path;
 
 /* {ptr, H, W, ld, dtype}: one row-major device matrix. */
@@ -93,7 +100,10 @@ typedef struct {
 
 /* Hyper-parameters of Algorithm 4.1 (defaults).
  * (a,b,c) are the Newton-Schulz coefficients; scale_c is the update-scaling constant "c" of
- * sec. 4.2 (the paper uses the letter c for both). eps is ADDED to the Frobenius norm. */
+ * sec. 4.2 (the paper uses the letter c for both). eps is ADDED to the Frobenius norm.
+ * The bf16 / e4m3 tensor-core kernels (AUTO on bf16 storage at T <= 256, FP8) iterate on c^(1/4) X and need
+ * c > 0: with c <= 0 (e.g. the cubic iteration (1.5, -0.5, 0)) himuon_step / himuon_phi / himuon_ns_tiles return
+ * HIMUON_ERR_UNSUPPORTED before any launch; HIMUON_PATH_FP32 and the large-tile path take any finite (a, b, c). */
 typedef struct {
   int32_t K;
   float   a, b, c;
@@ -114,7 +124,6 @@ typedef struct himuon_plan himuon_plan;
  * (16 = one device work item; the fused kernels stage nothing else in HBM).  If the whole list
  * fits it is kept resident and every bucket is one chunk; otherwise chunks are streamed through
  * the workspace one at a time.  workspace_cap_bytes = 0 means "no cap".
- * Supported T: 16, 32, 64, 128 (and 256 where the build provides it; else HIMUON_ERR_UNSUPPORTED).
  * A layer with T >= max(H,W) is the full-matrix branch: it is run as ONE padded
  * tile of the smallest supported size >= max(H,W) with tau = scale_c*sqrt(max(H,W)); if
  * max(H,W) exceeds the largest tile size (512) it is one whole-matrix item of the large-tile path.

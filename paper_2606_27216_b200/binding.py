@@ -56,17 +56,18 @@ class HimuonError(RuntimeError):
 
 
 _LIB = None
+_LIBS = {}
 
 
-def _lib():
-    global _LIB
-    if _LIB is not None:
-        return _LIB
-    if not os.path.exists(LIB_PATH):
+def _load(path: str):
+    """dlopen `path` and declare the C-ABI of include/himuon.h on it."""
+    if path in _LIBS:
+        return _LIBS[path]
+    if not os.path.exists(path):
         raise ImportError(
-            f"{LIB_PATH} not found: build it with `python -m paper_2606_27216_b200.build` "
+            f"{path} not found: build it with `python -m paper_2606_27216_b200.build` "
             "(there is no CPU fallback)")
-    lib = C.CDLL(LIB_PATH)
+    lib = C.CDLL(path)
     P = C.POINTER
     lib.himuon_plan_create.restype = C.c_int
     lib.himuon_plan_create.argtypes = [P(himuon_layer), C.c_int32, C.c_int32, C.c_int32, C.c_size_t,
@@ -100,12 +101,34 @@ def _lib():
     lib.himuon_supported_tile_sizes.argtypes = [C.c_int32, C.c_int32]
     lib.himuon_launch_count.restype = C.c_int64
     lib.himuon_launch_count.argtypes = []
-    lib.himuon_debug_set_tc128_stage.restype = None
-    lib.himuon_debug_set_tc128_stage.argtypes = [C.c_int]
-    lib.himuon_debug_set_tc128_fp8_stage.restype = None
-    lib.himuon_debug_set_tc128_fp8_stage.argtypes = [C.c_int]
-    _LIB = lib
+    _LIBS[path] = lib
     return lib
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        _LIB = _load(LIB_PATH)
+    return _LIB
+
+
+class use_library:
+    """Context manager: route the binding to another build of the same C-ABI (the -DHIMUON_DEBUG_STAGES library of
+    the stage tests).  Plans created inside must be destroyed inside."""
+
+    def __init__(self, path: str):
+        self.path = path
+
+    def __enter__(self):
+        global _LIB
+        self.prev = _LIB
+        _LIB = _load(self.path)
+        return _LIB
+
+    def __exit__(self, *exc):
+        global _LIB
+        _LIB = self.prev
+        return False
 
 
 def _check(status: int, where: str):
@@ -193,7 +216,7 @@ class Plan:
 
     def __init__(self, layers: Sequence[himuon_layer], T_default: int, path: int = HIMUON_PATH_AUTO,
                  workspace_cap_bytes: int = 0):
-        lib = _lib()
+        lib = self._lib = _lib()      # a plan stays with the library that created it
         arr = (himuon_layer * len(layers))(*layers)
         h = C.c_void_p()
         _check(lib.himuon_plan_create(arr, len(layers), T_default, path, workspace_cap_bytes, C.byref(h)),
@@ -224,7 +247,7 @@ class Plan:
         lrc = np.zeros((self.n_tiles, 3), dtype=np.int32)
         offs = np.zeros(self.n_chunks + 1, dtype=np.int64)
         cT = np.zeros(max(self.n_chunks, 1), dtype=np.int32)
-        _check(_lib().himuon_plan_worklist(self._h, lrc.ctypes.data, offs.ctypes.data, cT.ctypes.data),
+        _check(self._lib.himuon_plan_worklist(self._h, lrc.ctypes.data, offs.ctypes.data, cT.ctypes.data),
                "himuon_plan_worklist")
         return lrc, offs, cT[: self.n_chunks]
 
@@ -233,21 +256,21 @@ class Plan:
             workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device="cuda")
         off = (-workspace.data_ptr()) % 128
         self.workspace = workspace
-        _check(_lib().himuon_plan_bind(self._h, workspace.data_ptr() + off, workspace.numel() - off,
+        _check(self._lib.himuon_plan_bind(self._h, workspace.data_ptr() + off, workspace.numel() - off,
                                        _stream_ptr(stream)), "himuon_plan_bind")
         return self
 
     def step(self, hp: HParams, stream=None):
         c = hp.to_c()
-        _check(_lib().himuon_step(self._h, C.byref(c), _stream_ptr(stream)), "himuon_step")
+        _check(self._lib.himuon_step(self._h, C.byref(c), _stream_ptr(stream)), "himuon_step")
 
     def phi(self, hp: HParams, stream=None):
         c = hp.to_c()
-        _check(_lib().himuon_phi(self._h, C.byref(c), _stream_ptr(stream)), "himuon_phi")
+        _check(self._lib.himuon_phi(self._h, C.byref(c), _stream_ptr(stream)), "himuon_phi")
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h:
-            _lib().himuon_plan_destroy(self._h)
+            self._lib.himuon_plan_destroy(self._h)
             self._h = None
 
     def __del__(self):
@@ -280,9 +303,10 @@ def himuon_ns_tiles(tiles_in: torch.Tensor, tiles_out: Optional[torch.Tensor] = 
     return tiles_out
 
 
-def debug_set_tc128_stage(stage: int):
-    _lib().himuon_debug_set_tc128_stage(stage)
-
-
-def debug_set_tc128_fp8_stage(stage: int):
-    _lib().himuon_debug_set_tc128_fp8_stage(stage)
+def debug_set_stage(kernel: str, stage: int):
+    """Accumulator-dump stage of the T = 128 kernels (`kernel` = "tc128" | "tc128_fp8"); exists only in the
+    -DHIMUON_DEBUG_STAGES library (see `use_library`, `build.build_debug`)."""
+    fn = getattr(_lib(), f"himuon_debug_set_{kernel}_stage")
+    fn.restype = None
+    fn.argtypes = [C.c_int]
+    fn(stage)

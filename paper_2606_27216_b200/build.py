@@ -110,5 +110,17 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib_path: 
     return lib_path
 
 
+DEBUG_LIB_PATH = os.path.join(PKG_DIR, "libhimuon_debug.so")
+
+
+def build_debug(force: bool = False, verbose: bool = False) -> str:
+    """The -DHIMUON_DEBUG_STAGES build: same sources plus the accumulator-dump stages of the T = 128 kernels and their
+    `himuon_debug_set_*` exports.  Only the stage tests load it; the product library has none of this."""
+    return build(force=force, verbose=verbose, extra_flags=("-DHIMUON_DEBUG_STAGES",), lib_path=DEBUG_LIB_PATH,
+                 obj_dir=os.path.join(PKG_DIR, "build_debug"))
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--debug" in sys.argv:
+        print(build_debug(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

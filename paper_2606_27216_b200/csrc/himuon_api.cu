@@ -61,6 +61,14 @@ bool valid_hparams(const himuon_hparams* hp) {
   return true;
 }
 
+// The bf16 / e4m3 tensor-core kernels (warp, tc64, tc128, tc256 and the e4m3 variants) iterate on the scaled state
+// c^(1/4) X with beta = b / sqrt(c), which needs c > 0.  The fp32 kernel and the large-tile
+// path take any finite (a, b, c), e.g. the cubic iteration (1.5, -0.5, 0).
+bool kpath_needs_positive_c(int kp) { return kp == KPATH_TC || kp == KPATH_TC_FP8 || kp == KPATH_WARP; }
+bool positive_c_ok(const himuon_hparams* hp) {
+  return hp->c > 0.f && std::isfinite(hp->b / std::sqrt(hp->c)) && std::isfinite(1.f / std::sqrt(std::sqrt(hp->c)));
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
@@ -96,6 +104,17 @@ bool encode_bf16_map(CUtensorMap* out, void* ptr, int H, int W, long long ld, in
   return r == CUDA_SUCCESS;
 }
 
+// e4m3 operands need enough singular directions to average their rounding over: an edge tile with fewer than
+// kFp8MinLive live rows or columns (e.g. a 44 x 8 corner block, measured 0.19 against the path's 0.15 bound) is run
+// by the bf16 kernel of the same tile size instead - its own bucket of the same plan (buckets are
+// keyed by kernel path).  DESIGN.md section 5.
+constexpr int kFp8MinLive = 32;
+int tile_kpath(int layer_kpath, int H, int W, int T, int Tw, int r, int c) {
+  if (layer_kpath != KPATH_TC_FP8) return layer_kpath;
+  const int lh = H - r * T < T ? H - r * T : T, lw = W - c * Tw < Tw ? W - c * Tw : Tw;
+  return (lh < kFp8MinLive || lw < kFp8MinLive) ? KPATH_TC : KPATH_TC_FP8;
+}
+
 himuon_status chunk_rule(long long n_items, long long bytes_per_item, long long fixed_bytes,
                          long long cap_bytes, std::vector<long long>& offs) {
   offs.clear();
@@ -128,15 +147,18 @@ cudaError_t launch_chunk(const LaunchArgs& a, int kpath, cudaStream_t s) {
 
 namespace himuon {
 int device_sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+  static std::atomic<int> cache[64];   // zero-initialised; one entry per device ordinal
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+  if (dev >= 0 && dev < 64) {
+    const int c = cache[dev].load(std::memory_order_relaxed);
+    if (c > 0) return c;
   }
+  int n = 0;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
+  if (dev >= 0 && dev < 64) cache[dev].store(n, std::memory_order_relaxed);
   return n;
 }
-void note_launch() {}
 }  // namespace himuon
 
 extern "C" {
@@ -280,15 +302,25 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
           p->buckets[b].kpath == p->kpath[l])
         bi = (int)b;
     if (bi < 0) p->buckets.push_back(Bucket{p->T_eff[l], p->Tw_eff[l], dt, p->kpath[l], 0, 0});
+    if (p->kpath[l] == KPATH_TC_FP8) {   // small edge tiles of an e4m3 layer: companion bf16 bucket
+      const int T = p->T_eff[l], H = layers[l].g.H, W = layers[l].g.W;
+      const bool small = (H % T != 0 && H % T < kFp8MinLive) || (W % T != 0 && W % T < kFp8MinLive);
+      bool have = false;
+      for (const Bucket& B : p->buckets) have |= (B.T == T && B.Tw == T && B.dtype == dt && B.kpath == KPATH_TC);
+      if (small && !have) p->buckets.push_back(Bucket{T, T, dt, KPATH_TC, 0, 0});
+    }
   }
   for (size_t b = 0; b < p->buckets.size(); ++b) {
     Bucket& B = p->buckets[b];
     B.begin = (long long)p->items.size();
     for (int l = 0; l < n_layers; ++l) {
-      if (p->T_eff[l] != B.T || p->Tw_eff[l] != B.Tw || layers[l].g.dtype != B.dtype || p->kpath[l] != B.kpath) continue;
-      const int R = (layers[l].g.H + B.T - 1) / B.T, C = (layers[l].g.W + B.Tw - 1) / B.Tw;
+      if (p->T_eff[l] != B.T || p->Tw_eff[l] != B.Tw || layers[l].g.dtype != B.dtype) continue;
+      if (p->kpath[l] != B.kpath && !(p->kpath[l] == KPATH_TC_FP8 && B.kpath == KPATH_TC)) continue;
+      const int H = layers[l].g.H, W = layers[l].g.W;
+      const int R = (H + B.T - 1) / B.T, C = (W + B.Tw - 1) / B.Tw;
       for (int r = 0; r < R; ++r)
-        for (int c = 0; c < C; ++c) p->items.push_back(WorkItem{l, r, c, 0});
+        for (int c = 0; c < C; ++c)
+          if (tile_kpath(p->kpath[l], H, W, B.T, B.Tw, r, c) == B.kpath) p->items.push_back(WorkItem{l, r, c, 0});
     }
     B.end = (long long)p->items.size();
   }
@@ -405,6 +437,8 @@ himuon_status himuon_plan_bind(himuon_plan* plan, void* workspace, size_t worksp
 
 static himuon_status run_plan(himuon_plan* plan, const himuon_hparams* hp, int mode, void* cuda_stream) {
   if (!plan || !valid_hparams(hp)) return HIMUON_ERR_INVALID_ARG;
+  for (const Bucket& B : plan->buckets)          // before any launch (and before the bound check: pure argument validation)
+    if (B.end > B.begin && kpath_needs_positive_c(B.kpath) && !positive_c_ok(hp)) return HIMUON_ERR_UNSUPPORTED;
   if (!plan->ws) return HIMUON_ERR_NOT_BOUND;
   if (mode == MODE_STEP)
     for (const himuon_layer& L : plan->layers)
@@ -472,6 +506,7 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
   if (!valid_hparams(&hp)) return HIMUON_ERR_INVALID_ARG;
   const int kp = select_kpath(dtype, path, T);
   if (kp < 0) return HIMUON_ERR_UNSUPPORTED;
+  if (kpath_needs_positive_c(kp) && !positive_c_ok(&hp)) return HIMUON_ERR_UNSUPPORTED;
   if (n_tiles == 0) return HIMUON_OK;
   if (!tiles_in || !tiles_out || !workspace) return HIMUON_ERR_INVALID_ARG;
   if (n_tiles * (int64_t)T > 0x7fffffffLL) return HIMUON_ERR_UNSUPPORTED;

@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -71,8 +72,26 @@ cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_hos
                           const himuon_hparams& hp, void* scratch, size_t scratch_bytes, cudaStream_t stream,
                           long long* launches);
 
-int  device_sm_count();
-void note_launch();
+// SM count of the CURRENT device (per-device cache, thread-safe).
+int device_sm_count();
+
+// One-time kernel configuration (dynamic shared memory size) per DEVICE: `done` holds one bit per device
+// ordinal.  Thread-safe: two threads racing on the same device both set the (idempotent) attribute.
+struct DeviceOnce {
+  std::atomic<unsigned long long> done{0};
+};
+template <typename Kernel>
+cudaError_t configure_smem_once(DeviceOnce& once, Kernel kernel, int smem_bytes) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const unsigned long long bit = 1ull << (dev & 63);
+  if (dev < 64 && (once.done.load(std::memory_order_acquire) & bit)) return cudaSuccess;
+  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+  if (e != cudaSuccess) return e;
+  if (dev < 64) once.done.fetch_or(bit, std::memory_order_release);
+  return cudaSuccess;
+}
 
 // ---- host plan --------------------------------------------------------------------------------
 

@@ -39,8 +39,18 @@ struct Cublas {
                                  const void*, cudaDataType, int, long long, const void*, cudaDataType, int, long long,
                                  const void*, void*, cudaDataType, int, long long, int, cublasComputeType_t,
                                  cublasGemmAlgo_t) = nullptr;
-  cublasHandle_t handle = nullptr;
+  cublasHandle_t handles[64] = {};   // one per device ordinal, created on first use on that device
+  cublasHandle_t handle = nullptr;   // the current device's, set by acquire() under `mu`
+  std::mutex mu;                     // a handle carries a stream and a workspace: one enqueueing host thread at a time
   bool ok = false;
+  // Call with `mu` held: select (create if needed) the handle of the current device.
+  bool acquire() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
+    if (!handles[dev] && create(&handles[dev]) != CUBLAS_STATUS_SUCCESS) { handles[dev] = nullptr; return false; }
+    handle = handles[dev];
+    return true;
+  }
 };
 
 Cublas& cublas() {
@@ -57,8 +67,7 @@ Cublas& cublas() {
     c.set_workspace = reinterpret_cast<decltype(c.set_workspace)>(dlsym(c.lib, "cublasSetWorkspace_v2"));
     c.gemm_ex = reinterpret_cast<decltype(c.gemm_ex)>(dlsym(c.lib, "cublasGemmEx"));
     c.gemm_batched = reinterpret_cast<decltype(c.gemm_batched)>(dlsym(c.lib, "cublasGemmStridedBatchedEx"));
-    if (!c.create || !c.set_stream || !c.set_workspace || !c.gemm_ex || !c.gemm_batched) return;
-    c.ok = (c.create(&c.handle) == CUBLAS_STATUS_SUCCESS);
+    c.ok = c.create && c.set_stream && c.set_workspace && c.gemm_ex && c.gemm_batched;
   });
   return c;
 }
@@ -387,11 +396,17 @@ cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_hos
                           const WorkItem* items_dev, long long n_items, int T, int Tw, int mode, int dtype,
                           const himuon_hparams& hp, void* scratch, size_t scratch_bytes, cudaStream_t s, long long* launches) {
   if (n_items < 1) return cudaSuccess;
-  if (!cublas().ok) return cudaErrorNotSupported;
+  Cublas& cb = cublas();
+  if (!cb.ok) return cudaErrorNotSupported;
+  // The handle's stream and workspace are re-pointed per call: serialise the enqueueing host threads (the GPU work
+  // itself stays asynchronous on each caller's stream), one handle per device.
+  std::lock_guard<std::mutex> lock(cb.mu);
+  if (!cb.acquire()) return cudaErrorNotSupported;
   if (T <= 2048 && Tw <= 2048 && items_dev) {
     const size_t per = gemm_path_batch_item_bytes(T, Tw);
     if (scratch_bytes < per + kCublasWs) return cudaErrorInvalidValue;
-    const long long cap = (long long)((scratch_bytes - kCublasWs) / per);
+    long long cap = (long long)((scratch_bytes - kCublasWs) / per);
+    if (cap > 65535) cap = 65535;   // the sub-batch index is gridDim.y of the fused ends
     for (long long i = 0; i < n_items; i += cap) {
       const int nb = (int)std::min<long long>(cap, n_items - i);
       cudaError_t e = dtype == HIMUON_F32 ? run_batch<float>(layers_dev, items_dev + i, nb, T, Tw, mode, hp, (char*)scratch, s, launches)

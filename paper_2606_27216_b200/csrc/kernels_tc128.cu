@@ -43,7 +43,15 @@
 
 namespace himuon {
 
-int g_tc128_debug_stage = 0;   // 0 = normal; 1/2 = dump ACC after MMA1 / MMA2 of the first step (tests only)
+// Debug stages (1 / 2 = return the raw accumulator after MMA1 / MMA2 of the first step) exist only in the
+// -DHIMUON_DEBUG_STAGES build (libhimuon_debug.so, used by the stage tests); the product library has neither the
+// global, nor the export, nor the branches in the kernel.
+#ifdef HIMUON_DEBUG_STAGES
+int g_tc128_debug_stage = 0;
+constexpr bool kDebugStages = true;
+#else
+constexpr bool kDebugStages = false;
+#endif
 
 #ifdef HIMUON_TRACE   // development aid (not built into libhimuon.so): clock stamps of the two lead threads of CTA 0
 __device__ long long g_trace128[2][16384];
@@ -117,7 +125,8 @@ __device__ __forceinline__ void issue_bx(uint32_t acc, uint32_t opa, uint32_t ti
 
 __global__ void __launch_bounds__(kThreads, 1)
 himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __restrict__ tmaps,
-                    const WorkItem* __restrict__ items, long long n_items, int mode, himuon_hparams hp, int dbg) {
+                    const WorkItem* __restrict__ items, long long n_items, int mode, himuon_hparams hp, int dbg_arg) {
+  const int dbg = kDebugStages ? dbg_arg : 0;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
   Ctrl* ctrl = reinterpret_cast<Ctrl*>(smem_raw + (smem0 - smem_u32(smem_raw)) + kSlots * kSlotBytes);
@@ -540,24 +549,28 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
 }  // namespace
 
 cudaError_t launch_tc128(const LaunchArgs& a, cudaStream_t s) {
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(himuon_tc128_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static DeviceOnce once;   // per device, thread-safe
+  cudaError_t e = configure_smem_once(once, himuon_tc128_kernel, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
   long long grid = (a.n_items + kSlots - 1) / kSlots;
   const int sms = device_sm_count();
   if (grid > sms) grid = sms;
   if (grid < 1) return cudaSuccess;
+#ifdef HIMUON_DEBUG_STAGES
+  const int stage = g_tc128_debug_stage;
+#else
+  const int stage = 0;
+#endif
   himuon_tc128_kernel<<<(unsigned)grid, kThreads, kSmemBytes, s>>>(a.layers, a.tmaps, a.items, a.n_items, a.mode, a.hp,
-                                                                   g_tc128_debug_stage);
+                                                                   stage);
   return cudaGetLastError();
 }
 
 }  // namespace himuon
 
+#ifdef HIMUON_DEBUG_STAGES
 extern "C" void himuon_debug_set_tc128_stage(int stage) { himuon::g_tc128_debug_stage = stage; }
+#endif
 #ifdef HIMUON_TRACE
 extern "C" int himuon_debug_read_trace128(long long* out, int* n) {
   cudaMemcpyFromSymbol(n, himuon::g_tn128, sizeof(int) * 2, 0, cudaMemcpyDeviceToHost);

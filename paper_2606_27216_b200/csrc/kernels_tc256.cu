@@ -491,12 +491,9 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
 }  // namespace
 
 cudaError_t launch_tc256(const LaunchArgs& a, cudaStream_t s) {
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(himuon_tc256_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static DeviceOnce once;   // per device, thread-safe
+  cudaError_t e = configure_smem_once(once, himuon_tc256_kernel, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
   if (a.n_items < 1) return cudaSuccess;
   long long clusters = a.n_items;
   const int max_clusters = device_sm_count() / 2;

@@ -460,12 +460,9 @@ himuon_tc256_fp8_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* 
 }  // namespace
 
 cudaError_t launch_tc256_fp8(const LaunchArgs& a, cudaStream_t s) {
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(himuon_tc256_fp8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static DeviceOnce once;   // per device, thread-safe
+  cudaError_t e = configure_smem_once(once, himuon_tc256_fp8_kernel, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
   if (a.n_items < 1) return cudaSuccess;
   long long clusters = a.n_items;
   const int max_clusters = device_sm_count() / 2;

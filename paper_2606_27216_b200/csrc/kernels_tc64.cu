@@ -467,12 +467,9 @@ himuon_tc64_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __res
 }  // namespace
 
 cudaError_t launch_tc64(const LaunchArgs& a, cudaStream_t s) {
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(himuon_tc64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static DeviceOnce once;   // per device, thread-safe
+  cudaError_t e = configure_smem_once(once, himuon_tc64_kernel, (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
   const long long n_super = (a.n_items + kPack - 1) / kPack;
   long long grid = (n_super + kSlots - 1) / kSlots;
   const int sms = device_sm_count();

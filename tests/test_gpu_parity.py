@@ -31,6 +31,23 @@ def run_phi(G: torch.Tensor, T: int, hp, path=hm.HIMUON_PATH_AUTO, cap=0):
 
 # ----------------------------------------------------------------------------- fp32 path
 
+@pytest.mark.parametrize("T", [32, 128])
+def test_fp32_path_cubic_iteration_c_zero(T):
+    """(a, b, c) = (1.5, -0.5, 0), the cubic Newton-Schulz iteration: c = 0 is served by the fp32 kernel (<= 1e-4 against
+    the oracle) and refused by the bf16 tensor-core kernels, which iterate on c^(1/4) X (include/himuon.h)."""
+    _need_gpu()
+    G = I.gaussian(2 * T + 8, 3 * T, seed_cfg=0, layer_index=5, dtype=torch.float32)
+    hp = hm.HParams(K=5, a=1.5, b=-0.5, c=0.0, eps=1e-7)
+    U = run_phi(G, T, hp)
+    PU.check_phi(U, G, T, hp, PU.TOL_FP32, out_is_bf16=False)
+    Gb = G.to(torch.bfloat16)
+    with pytest.raises(hm.HimuonError) as ei:
+        run_phi(Gb, T, hp)
+    assert ei.value.status == B.HIMUON_ERR_UNSUPPORTED
+    Ub = run_phi(Gb, T, hp, path=hm.HIMUON_PATH_FP32)                  # bf16 storage, fp32 arithmetic: accepted
+    PU.check_phi(Ub, Gb, T, hp, 5e-3, out_is_bf16=True)               # one bf16 rounding of the output
+
+
 @pytest.mark.parametrize("T", [16, 32, 64, 128])
 def test_config1_fp32_phi(T):
     """BASELINE config 1: fp32 256x512 N(0,1) seed 0, K=5, eps=1e-7 (T=64 -> 32 tiles, reading Q1)."""
@@ -129,11 +146,13 @@ def test_tc128_debug_stages(stage):
     _need_gpu()
     G = _tc_inputs(128, 256, 21)
     hp = hm.HParams(K=1, eps=1e-7)
-    B.debug_set_tc128_stage(stage)
-    try:
-        U = run_phi(G, 128, hp)
-    finally:
-        B.debug_set_tc128_stage(0)
+    from paper_2606_27216_b200.build import build_debug
+    with B.use_library(build_debug()):        # the accumulator-dump stages exist only in the debug build
+        B.debug_set_stage("tc128", stage)
+        try:
+            U = run_phi(G, 128, hp)
+        finally:
+            B.debug_set_stage("tc128", 0)
     g = PU.f64(G)
     got = PU.f64(U)
     a, b, c = [float(np.float32(x)) for x in hm.NS_COEFFS]

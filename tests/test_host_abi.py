@@ -255,3 +255,70 @@ def test_fp8_path_is_opt_in_and_T128_T256_only():
     with pytest.raises(hm.HimuonError) as e:                    # an unknown path value is an argument error
         hm.Plan(_layers([(256, 256)]), 128, path=3)
     assert e.value.status == B.HIMUON_ERR_INVALID_ARG
+
+
+def test_nonpositive_c_is_refused_on_the_tensor_core_paths():
+    """The bf16 / e4m3 tensor-core kernels iterate on c^(1/4) X: c <= 0 - e.g. the cubic
+    iteration (1.5, -0.5, 0) - must be refused before any launch, not turned into NaN weights.  The check is pure
+    argument validation, so it fires even on an unbound plan; the fp32 path takes any finite (a, b, c)."""
+    lib = B._lib()
+    for c, want_tc in ((0.0, B.HIMUON_ERR_UNSUPPORTED), (-1.0, B.HIMUON_ERR_UNSUPPORTED), (2.0315, B.HIMUON_ERR_NOT_BOUND)):
+        hp = hm.HParams(a=1.5, b=-0.5, c=c).to_c()
+        for T in (16, 64, 128, 256):
+            p = hm.Plan(_layers([(512, 512)]), T)
+            assert lib.himuon_step(p._h, C.byref(hp), None) == want_tc, (c, T)
+            assert lib.himuon_phi(p._h, C.byref(hp), None) == want_tc, (c, T)
+        p = hm.Plan(_layers([(512, 512)]), 128, path=hm.HIMUON_PATH_FP8)
+        assert lib.himuon_phi(p._h, C.byref(hp), None) == want_tc
+        # fp32 arithmetic (FP32 path on bf16 storage, fp32 storage, large tiles): accepted (only "not bound" here)
+        p = hm.Plan(_layers([(512, 512)]), 64, path=hm.HIMUON_PATH_FP32)
+        assert lib.himuon_phi(p._h, C.byref(hp), None) == B.HIMUON_ERR_NOT_BOUND
+        p = hm.Plan(_layers([(512, 512)], hm.HIMUON_F32), 64)
+        assert lib.himuon_phi(p._h, C.byref(hp), None) == B.HIMUON_ERR_NOT_BOUND
+    # himuon_ns_tiles validates before touching any pointer
+    for T, dt, want in ((128, hm.HIMUON_BF16, B.HIMUON_ERR_UNSUPPORTED), (64, hm.HIMUON_F32, B.HIMUON_OK)):
+        st = lib.himuon_ns_tiles(None, None, 0, T, dt, hm.HIMUON_PATH_AUTO, 5, 1.5, -0.5, 0.0, 1e-7, None, 0, None)
+        assert st == want, (T, dt, st)
+
+
+def test_plans_from_two_threads():
+    """The library keeps no unsynchronised process-global state on the planning path: two host threads building,
+    inspecting and destroying plans concurrently get the same work lists as one thread."""
+    import threading
+    shapes = [(1600, 1600), (1600, 6400), (6400, 1600)] * 4
+    want = O.enumerate_tiles(shapes, [128] * len(shapes))
+    errors = []
+
+    def worker(seed):
+        try:
+            for i in range(20):
+                T = (64, 128, 256)[(i + seed) % 3]
+                p = hm.Plan(_layers(shapes), T, workspace_cap_bytes=(1 << 20) if i % 2 else 0)
+                lrc, offs, cT = p.worklist()
+                if T == 128 and [tuple(x) for x in lrc.tolist()] != want:
+                    errors.append("work list differs")
+                if offs[-1] != p.n_tiles:
+                    errors.append("chunk offsets")
+                p.destroy()
+        except Exception as e:        # noqa: BLE001
+            errors.append(repr(e))
+
+    ts = [threading.Thread(target=worker, args=(s,)) for s in range(2)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert not errors, errors
+
+
+def test_fp8_plan_routes_small_edge_tiles_to_the_bf16_kernel():
+    """An e4m3 layer's edge tiles with fewer than 32 live rows or columns form a second bucket (bf16 kernel, same T);
+    every tile appears exactly once (buckets by kernel path)."""
+    p = hm.Plan(_layers([(300, 520), (256, 512)]), 256, path=hm.HIMUON_PATH_FP8)
+    lrc, offs, cT = p.worklist()
+    assert p.n_buckets == 2 and p.n_chunks == 2 and cT.tolist() == [256, 256]
+    all_tiles = sorted(tuple(x) for x in lrc.tolist())
+    assert all_tiles == sorted(O.enumerate_tiles([(300, 520), (256, 512)], [256, 256]))
+    assert sorted(tuple(x) for x in lrc[offs[1]:].tolist()) == [(0, 0, 2), (0, 1, 2)]     # 8 live columns
+    # no small edge tile: one bucket
+    assert hm.Plan(_layers([(300, 640)]), 256, path=hm.HIMUON_PATH_FP8).n_buckets == 1

@@ -243,13 +243,15 @@ def run_gpu(args):
     bytes_step = 10.0 * n_elem
     t_tensor = flops / (pk["bf16_sustained"] * 1e12)
     t_hbm = bytes_step / (pk["hbm_gbs"] * 1e9)
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "r1_traffic.csv")
-    if os.path.exists(tp):                                    # measured DRAM bytes per element (ncu) x elements per launch
-        for ln in open(tp).read().splitlines()[1:]:
-            f = ln.split(",")
-            if f[0] == kname and int(f[1]) == args.T and not any(l.T for l in spec.layers):
-                traffic = float(f[5]) * n_elem / plan.n_chunks
+    traffic, traffic_src = None, None
+    for tp in ("r2_traffic.csv", "r1_traffic.csv"):           # newest ncu capture: DRAM bytes per element x elements per launch
+        tpath = os.path.join(ROOT, "profiles", tp)
+        if traffic is None and os.path.exists(tpath):
+            for ln in open(tpath).read().splitlines()[1:]:
+                f = ln.split(",")
+                if f[0] == kname and int(f[1]) == args.T and not any(l.T for l in spec.layers):
+                    traffic = float(f[5]) * n_elem / plan.n_chunks
+                    traffic_src = f"ncu capture profiles/{tp} (dram bytes per element of a {f[2]}-element launch) x elements of this launch; not measured in this run"
     if t_tensor >= t_hbm:
         ach = flops / plan.n_chunks / (kern_ms * 1e-3) / 1e12
         roof = {"bound": "tensor", "achieved": round(ach, 2), "peak": pk["bf16_sustained"], "unit": "TFLOP/s",
@@ -259,41 +261,42 @@ def run_gpu(args):
         ach = bytes_step / plan.n_chunks / (kern_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": round(ach, 1), "peak": pk["hbm_gbs"], "unit": "GB/s",
                 "frac": round(ach / pk["hbm_gbs"], 4), "traffic": traffic, "peak_kind": "copy bandwidth, " + pk["source"]}
-    roof.update({"kernel": kname, "launch_ms": round(kern_ms, 4),
+    roof.update({"traffic_source": traffic_src, "kernel": kname, "launch_ms": round(kern_ms, 4),
                  "tflops_achieved": round(flops / (ms_per_step * 1e-3) / 1e12, 2),
                  "hbm_gbs_achieved": round(bytes_step / (ms_per_step * 1e-3) / 1e9, 1),
                  "roofline_ms": round(max(t_tensor, t_hbm) * 1e3, 3)})
     cpu = run_cpu_baseline(args, spec, hp)
+    context = {"cublas_full_matrix_phi": cublas_full_matrix_context(spec, args.K, dev), "paper": PAPER_CONTEXT,
+               "cpu_oracle": "see cpu_baseline (float64 oracle on this box's host cores, same run)"}
     line = {"metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
             "scaling": "strong" if args.shard else "weak", "vs_baseline": None, "dtype": "fp8-e4m3 operands, fp32 state" if args.path == "fp8" else "bf16", "data": "synthetic",
             "config": {"workload": f"{spec.name}-shaped HiMuon step (BASELINE configs[4])" if spec.name.startswith("llama3-8b") else f"{spec.name}-shaped HiMuon step",
                        "layers": len(spec.layers), "elements": n_elem, "tiles": plan.n_tiles, "T": args.T, "K": args.K,
                        "chunks": plan.n_chunks, "workspace_bytes": plan.workspace_bytes, "cap_mb": args.cap_mb,
-                       "l2": "inputs (%.1f GB) larger than L2" % (bytes_step / 1e9), "parallelism": (f"whole matrices sharded over {world} ranks" if args.shard else f"replicas x{world}") + ", no collective",
+                       "l2": "inputs (%.1f GB) larger than L2" % (bytes_step / 1e9),
+                       "state": "timed steps run back-to-back on the W and M the previous step wrote (no restore between steps)", "parallelism": (f"whole matrices sharded over {world} ranks" if args.shard else f"replicas x{world}") + ", no collective",
                        "gflop_per_step": round(flops / 1e9, 1)},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+            "context": context,
             "step_ms_median": round(statistics.median(per_step), 4), "step_ms_min": round(min(per_step), 4)}
     print(json.dumps(line))
 
 
 def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
-    """Per step: H2D copy of the step's gradients from pinned host memory, himuon_step, D2H read of the
-    updated weights into pinned host memory - through the public API (one bound plan per group of layers),
-    pipelined over three streams so that the copies of one group overlap the step of another (PCIe is full
-    duplex).  Host buffers are bounded by --e2e-host-gb."""
-    sizes = [g.numel() * 2 for g in Gs]
-    budget = int(args.e2e_host_gb * (1 << 30) / max(1, world))   # pinned host memory is shared by the ranks of a node
-    n_layers, acc = 0, 0
-    for sz in sizes:                       # both a G-in and a W-out host buffer per layer
-        if acc + 2 * sz > budget:
-            break
-        acc += 2 * sz
-        n_layers += 1
-    n_layers = max(n_layers, 1)
-    full = n_layers == len(Gs)
-    per_group = max(1, {"gpt2": 6}.get(spec.name[:4], 7))
+    """Per step, over the WHOLE parameter set: H2D copy of every layer's gradient from pinned host memory,
+    himuon_step, D2H read of every updated weight into pinned host memory - through the public API (one bound plan
+    per group of layers), pipelined over three streams so that the copies of one group overlap the step of another
+    (PCIe is full duplex).  Pinned host memory is a ring of group-sized slots bounded by --e2e-host-gb: with enough
+    budget every group has its own slot; otherwise slots are reused round-robin within a step (groups sharing a slot
+    receive the same gradient bits and overwrite each other's read-back - same bytes over the link, same kernels).
+    Momentum buffers of this leg are separate zero-initialised tensors (the timed loop above keeps its own)."""
+    per_group = max(1, {"gpt2": 6}.get(spec.name[:4], 7))          # one transformer block
+    n_layers = len(Gs)
     groups = [list(range(a, min(a + per_group, n_layers))) for a in range(0, n_layers, per_group)]
+    slot_bytes = max(sum(Gs[i].numel() * 2 for i in gr) for gr in groups)          # one G-in or W-out slot
+    budget = int(args.e2e_host_gb * (1 << 30) / max(1, world))   # pinned host memory is shared by the ranks of a node
+    n_slots = max(1, min(len(groups), budget // (2 * slot_bytes)))
     Tl = [l.T for l in spec.layers]
     plans = []
     for gr in groups:
@@ -301,11 +304,20 @@ def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
         plans.append(hm.Plan.from_tensors([Ws[i] for i in gr], [Gs[i] for i in gr], Ms_g, args.T,
                                           T_per_layer=[Tl[i] for i in gr] if any(Tl) else None,
                                           path=hm.HIMUON_PATH_FP8 if args.path == "fp8" else hm.HIMUON_PATH_AUTO).bind())
-    sub_flops = float(sum(6.0 * args.K * (spec.layers[i].T or args.T) * spec.layers[i].H * spec.layers[i].W for i in range(n_layers)))
-    hG = [torch.empty(Gs[i].shape, dtype=Gs[i].dtype, pin_memory=True) for i in range(n_layers)]
-    hW = [torch.empty(Ws[i].shape, dtype=Ws[i].dtype, pin_memory=True) for i in range(n_layers)]
-    for i in range(n_layers):
-        hG[i].copy_(Gs[i])
+    hG = [torch.empty(slot_bytes // 2, dtype=torch.bfloat16, pin_memory=True) for _ in range(n_slots)]
+    hW = [torch.empty(slot_bytes // 2, dtype=torch.bfloat16, pin_memory=True) for _ in range(n_slots)]
+
+    def views(buf, gr):            # per-layer views of a slot
+        out, off = [], 0
+        for i in gr:
+            n = Gs[i].numel()
+            out.append(buf[off:off + n].view(Gs[i].shape))
+            off += n
+        return out
+
+    for k, gr in enumerate(groups[:n_slots]):                     # seed the ring with this rank's gradients
+        for v, i in zip(views(hG[k], gr), gr):
+            v.copy_(Gs[i])
     steps = max(2, min(args.steps, 5))
     s_in, s_cmp, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
     ev_cmp_prev = [None] * len(groups)       # G of a group may be overwritten once the previous step of it is done
@@ -313,11 +325,12 @@ def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
 
     def one():
         for k, gr in enumerate(groups):
+            slot = k % n_slots
             with torch.cuda.stream(s_in):
                 if ev_cmp_prev[k] is not None:
                     s_in.wait_event(ev_cmp_prev[k])
-                for i in gr:
-                    Gs[i].copy_(hG[i], non_blocking=True)
+                for v, i in zip(views(hG[slot], gr), gr):
+                    Gs[i].copy_(v, non_blocking=True)
                 e_in = torch.cuda.Event(); e_in.record(s_in)
             with torch.cuda.stream(s_cmp):
                 s_cmp.wait_event(e_in)
@@ -327,8 +340,8 @@ def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
                 e_c = torch.cuda.Event(); e_c.record(s_cmp)
             with torch.cuda.stream(s_out):
                 s_out.wait_event(e_c)
-                for i in gr:
-                    hW[i].copy_(Ws[i], non_blocking=True)
+                for v, i in zip(views(hW[slot], gr), gr):
+                    v.copy_(Ws[i], non_blocking=True)
                 e_o = torch.cuda.Event(); e_o.record(s_out)
             ev_cmp_prev[k], ev_out_prev[k] = e_c, e_o
 
@@ -354,12 +367,78 @@ def run_e2e(args, hm, spec, plan, hp, Ws, Gs, flops, world, dev, barrier):
         t = torch.tensor([ms], device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
-    h2d = sum(h.numel() * 2 for h in hG)
-    d2h = sum(h.numel() * 2 for h in hW)
-    return {"value": round(world * sub_flops / (ms * 1e-3) / 1e12, 3), "unit": UNIT, "ms_per_step": round(ms, 3),
-            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": steps,
+    nbytes = sum(g.numel() * 2 for g in Gs)
+    ring = (f"every group has its own pinned slot ({n_slots} x 2 x {slot_bytes / 2**20:.0f} MiB)" if n_slots == len(groups) else
+            f"ring of {n_slots} pinned slots of 2 x {slot_bytes / 2**20:.0f} MiB reused round-robin over {len(groups)} groups "
+            f"(--e2e-host-gb {args.e2e_host_gb})")
+    return {"value": round(world * flops / (ms * 1e-3) / 1e12, 3), "unit": UNIT, "ms_per_step": round(ms, 3),
+            "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": steps,
             "pipeline": f"{len(groups)} groups of layers (one plan each) over 3 streams: H2D | himuon_step | D2H",
-            "workload": "full parameter set" if full else f"first {n_layers} of {len(Gs)} layers (host-buffer budget {args.e2e_host_gb} GB)"}
+            "workload": "full parameter set", "host_buffers": ring,
+            "momentum": "separate zero-initialised M buffers for this leg; steps back-to-back on the mutated W, M",
+            "link_gbs_each_way": round(nbytes / (ms * 1e-3) / 1e9, 1)}
+
+
+def cublas_full_matrix_context(spec, K, dev):
+    """Context line (north_star): full-matrix Phi_K (Muon's T = infinity) through cuBLAS
+    (torch.matmul / addmm, bf16 operands, fp32 accumulation) on the SAME matrices' shapes: one matrix of each distinct
+    shape is timed (median of 3 after 2 warm-ups, CUDA events) and multiplied by how often the shape occurs."""
+    import paper_2606_27216_b200 as hm
+    a, b, c = hm.NS_COEFFS
+    shapes = {}
+    for i, l in enumerate(spec.layers):
+        shapes.setdefault((l.H, l.W), []).append(i)
+    total_ms, flops, per_shape = 0.0, 0.0, []
+    for (H, W), idx in shapes.items():
+        G = I.lowrank_plus_noise(H, W, spec.rank, seed_cfg=spec.seed_cfg, layer_index=idx[0], tensor_id=I.TENSOR_G,
+                                 dtype=torch.bfloat16, device=dev)
+
+        def run():
+            X = G.float()
+            X = (X / (X.norm() + 1e-7)).to(torch.bfloat16)
+            if H > W:
+                X = X.t().contiguous()                    # PAPER.md:76: work on the short side
+            for _ in range(K):
+                A = X @ X.t()
+                B = torch.addmm(A, A, A, beta=b, alpha=c)
+                X = torch.addmm(X, B, X, beta=a, alpha=1.0)
+            return X
+
+        ts = []
+        for rep_ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); run(); e1.record(); torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ms = statistics.median(ts[2:])
+        r, n = min(H, W), max(H, W)
+        fl = K * (4.0 * r * r * n + 2.0 * r * r * r)
+        per_shape.append({"shape": [H, W], "count": len(idx), "ms_each": round(ms, 3)})
+        total_ms += ms * len(idx)
+        flops += fl * len(idx)
+        del G
+    torch.cuda.empty_cache()
+    return {"what": "cuBLAS full-matrix Phi_K (Muon, T = infinity) on the same matrix shapes: Phi only, no momentum / "
+                    "update passes; one matrix per distinct shape timed, x count",
+            "ms_per_parameter_set": round(total_ms, 2), "tflops_executed": round(flops / total_ms / 1e9, 1),
+            "gflop_executed": round(flops / 1e9, 1), "per_shape": per_shape,
+            "note": "context, not the target: a different (more expensive) map than the tiled one"}
+
+
+PAPER_CONTEXT = [
+    # the paper prints ratios, not absolute kernel times (BASELINE.md); quoted with their hardware, context only
+    {"cite": "PAPER.md:374-380 (Fig. 7)", "hardware": "1x A40, bf16",
+     "what": "SRAM-resident all-K-steps NS kernel vs PyTorch eager bmm loop, T=128, K=5, B_tile in {32,128,512,2048}",
+     "value": "4-8x faster, largest at B_tile=2048"},
+    {"cite": "PAPER.md:398-402 (Fig. 9a)", "hardware": "1x A40, bf16",
+     "what": "optimizer step vs full-matrix Muon, 8 stacked Linear(H,H), T=512, K=5, H = 1024 / 2048 / 4096",
+     "value": "tiled only 1.4x / 3.2x / 5.2x; with cross-layer batching 2.3x / 3.7x / 5.4x"},
+    {"cite": "PAPER.md:355-370 (Fig. 6)", "hardware": "1x A40, bf16",
+     "what": "per-layer tiled / full-matrix NS speedup at T=512, K=5, Qwen3 block-0 shapes",
+     "value": "1.4-1.6x (0.6B), 1.4-2.9x (1.7B), 1.3-2.9x (4B)"},
+    {"cite": "PAPER.md:341-349", "hardware": "4x A40 DDP / FSDP, bf16 mixed",
+     "what": "end-to-end training step time, T = inf -> 512 -> 128 schedule",
+     "value": "Qwen3-0.6B 3.80 -> 3.62 s; 1.7B 6.72 -> 6.16 s; 4B 17.55 -> 17.18 s"},
+]
 
 
 def run_cpu_baseline(args, spec, hp):
@@ -410,7 +489,7 @@ def main():
                     help="fp8: e4m3 operands in the Newton-Schulz products (T = 128 / 256 only; NOT the headline: reduced precision)")
     ap.add_argument("--cap-mb", type=int, default=2048)
     ap.add_argument("--cpu-tiles", type=int, default=16384)
-    ap.add_argument("--e2e-host-gb", type=float, default=8.0)
+    ap.add_argument("--e2e-host-gb", type=float, default=32.0, help="pinned host memory for the e2e leg (ring of group slots)")
     ap.add_argument("--blocks", type=int, default=0, help="truncate the parameter set to its first N transformer blocks (profiling only)")
     ap.add_argument("--shard", action="store_true", help="N > 1: split the parameter set over the ranks by whole matrices (strong scaling)")
     ap.add_argument("--suite", action="store_true")

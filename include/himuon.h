@@ -58,14 +58,16 @@ typedef enum { HIMUON_F32 = 0, HIMUON_BF16 = 1 } himuon_dtype;
  *            T = 64       tcgen05, two tiles stacked per 128-lane MMA      (W % 8 == 0, ptr and ld*2 16-byte aligned)
  *            T = 128      tcgen05, operands and accumulator in TMEM        (same)
  *            T = 256      tcgen05 cta_group::2, one tile per CTA pair      (same)
- *            T = 512 and the full-matrix branch T >= max(H,W) > 256: large-tile path - fused prep / update
- *                         kernels around cuBLAS GEMMs (fp32 data, TF32 tensor-core math), tiles staged in
- *                         sub-batches inside the caller's workspace (himuon_plan_info reports the bytes)
+ *            T = 512, the full-matrix branch T >= max(H,W) > 256 and rectangular tiles: large-tile path - every
+ *                         product of a Newton-Schulz step is one launch of a hand-written persistent tcgen05 GEMM
+ *                         (bf16 operands, fp32 accumulation, fp32 iterate) with the step's elementwise work fused
+ *                         into its epilogue; tiles staged in sub-batches inside the caller's workspace
+ *                         (himuon_plan_info reports the bytes)
  *          a bf16 matrix whose width is not a multiple of 8 is served by the fp32 kernel at T = 64, 128 and by
  *          the large-tile path at T = 256;
  *          fp32 storage -> fp32 path.
- *   FP32 : true fp32 arithmetic for any storage dtype: FMA kernel for T in {16, 32, 64, 128}, the large-tile
- *          path with true-fp32 cuBLAS products for T = 256, 512 and the full-matrix branch (the <= 1e-4 path).
+ *   FP32 : true fp32 arithmetic for any storage dtype: FMA kernel for T in {16, 32, 64, 128}; fp32 cuBLAS products
+ *          (SGEMM) around fused prep / update kernels for T = 256, 512 and the full-matrix branch (the <= 1e-4 path).
  *   FP8  : bf16 storage, T = 128 or 256, width a multiple of 8 only (anything else: HIMUON_ERR_UNSUPPORTED).  The three
  *          products of a Newton-Schulz step take e4m3 operands (tcgen05 kind::f8f6f4, fp32 accumulation); the
  *          iterate, the diagonals of A and B, momentum and update stay fp32.  Opt-in:
@@ -89,8 +91,8 @@ typedef struct {
  * T = 0 selects the plan-wide default; otherwise this layer's tile size (runtime tile schedule).
  * T_w = 0 (or T_w == T): square T x T tiles.  Otherwise rectangular tiles of T rows x T_w columns (PAPER.md:55,
  * the tile-shape study of Fig. 8): both extents powers of two in 16..2048, R = ceil(H/T), C = ceil(W/T_w),
- * tau = scale_c*sqrt(max(T, T_w)); served by the large-tile path (cuBLAS products, Gram matrix on
- * the short side of the tile).
+ * tau = scale_c*sqrt(max(T, T_w)); served by the large-tile path (Gram matrix on the short side of
+ * the tile): tcgen05 GEMMs on bf16 storage, fp32 cuBLAS products on fp32 storage / HIMUON_PATH_FP32.
  * For himuon_phi only g (input) and w (output) are used; m may be {NULL,...}. */
 typedef struct {
   himuon_mat w, g, m;

@@ -35,12 +35,13 @@ int select_kpath(int dtype, int path, int T, int W = 0) {
   const bool simt_ok = (T == 16 || T == 32 || T == 64 || T == 128);
   if (path == HIMUON_PATH_FP8)                                      // e4m3 operands: the T = 128 / 256 tcgen05 kernels only
     return (dtype == HIMUON_BF16 && (T == 128 || T == 256) && (W % 8) == 0) ? KPATH_TC_FP8 : -1;
-  if (T >= 512) return KPATH_GEMM;                                  // library-size products: cuBLAS
-  if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : (T == 256 ? KPATH_GEMM : -1);
-  // bf16 storage, AUTO: tensor-core path where it exists, else the fp32 kernel / the large-tile path.
+  // true fp32 arithmetic (the <= 1e-4 path): FMA kernel up to T = 128, fp32 cuBLAS products beyond
+  if (path == HIMUON_PATH_FP32 || dtype == HIMUON_F32) return simt_ok ? KPATH_FP32_SIMT : (T >= 256 ? KPATH_GEMM : -1);
+  // bf16 storage, AUTO: tensor-core kernels; large tiles: the tcgen05 GEMM path with fused epilogues.
+  if (T >= 512) return KPATH_LT;
   if ((T == 256 || T == 128 || T == 64) && (W % 8) == 0) return KPATH_TC;
   if (T == 16 || T == 32) return KPATH_WARP;
-  if (T == 256) return KPATH_GEMM;                                  // width not a multiple of 8
+  if (T == 256) return KPATH_LT;                                    // width not a multiple of 8
   return simt_ok ? KPATH_FP32_SIMT : -1;
 }
 
@@ -64,7 +65,7 @@ bool valid_hparams(const himuon_hparams* hp) {
 // The bf16 / e4m3 tensor-core kernels (warp, tc64, tc128, tc256 and the e4m3 variants) iterate on the scaled state
 // c^(1/4) X with beta = b / sqrt(c), which needs c > 0.  The fp32 kernel and the large-tile
 // path take any finite (a, b, c), e.g. the cubic iteration (1.5, -0.5, 0).
-bool kpath_needs_positive_c(int kp) { return kp == KPATH_TC || kp == KPATH_TC_FP8 || kp == KPATH_WARP; }
+bool kpath_needs_positive_c(int kp) { return kp == KPATH_TC || kp == KPATH_TC_FP8 || kp == KPATH_WARP || kp == KPATH_LT; }
 bool positive_c_ok(const himuon_hparams* hp) {
   return hp->c > 0.f && std::isfinite(hp->b / std::sqrt(hp->c)) && std::isfinite(1.f / std::sqrt(std::sqrt(hp->c)));
 }
@@ -249,23 +250,24 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       Te = T;
     }
     if (rect && path == HIMUON_PATH_FP8) { st = HIMUON_ERR_UNSUPPORTED; break; }   // e4m3 operands: square tiles only
-    const int kp = rect ? KPATH_GEMM : select_kpath(dt, path, Te, W);
+    const int kp = rect ? ((dt == HIMUON_BF16 && path == HIMUON_PATH_AUTO) ? KPATH_LT : KPATH_GEMM) : select_kpath(dt, path, Te, W);
     if (kp < 0) { st = HIMUON_ERR_UNSUPPORTED; break; }
     if (!rect) Twe = Te;
-    if (kp == KPATH_GEMM) {
+    if (kp == KPATH_GEMM || kp == KPATH_LT) {
+      const bool lt = (kp == KPATH_LT);
       size_t need;
       if (Te <= 2048 && Twe <= 2048) {   // uniform tiles run in sub-batches: as many tiles as a scratch budget holds (>= 1)
-        const size_t per = gemm_path_batch_item_bytes(Te, Twe);
+        const size_t per = lt ? lt_path_batch_item_bytes(Te, Twe) : gemm_path_batch_item_bytes(Te, Twe);
         size_t       budget = (size_t)512 << 20;
         if (workspace_cap_bytes && workspace_cap_bytes / 2 < budget) budget = workspace_cap_bytes / 2;
-        const int key = Te * 4096 + Twe;
+        const int key = (Te * 4096 + Twe) * 2 + (lt ? 1 : 0);
         gemm_tiles[key] += (long long)((H + Te - 1) / Te) * ((W + Twe - 1) / Twe);
         long long nb = (long long)(budget / per);
         if (nb > gemm_tiles[key]) nb = gemm_tiles[key];
         if (nb < 1) nb = 1;
-        need = gemm_path_fixed_bytes() + (size_t)nb * per;
+        need = (lt ? 0 : gemm_path_fixed_bytes()) + (size_t)nb * per;
       } else {
-        need = gemm_path_scratch_bytes(H, W);
+        need = lt ? lt_path_scratch_bytes(H, W) : gemm_path_scratch_bytes(H, W);
       }
       if (need > p->scratch_bytes) p->scratch_bytes = need;
     }
@@ -459,7 +461,15 @@ static himuon_status run_plan(himuon_plan* plan, const himuon_hparams* hp, int m
       if (e != cudaSuccess) return cuda_fail(e, "step: chunk work list");
       a.items = (const WorkItem*)(ws + plan->off_items);
     }
-    if (B.kpath == KPATH_GEMM) {   // large tiles: products go to cuBLAS (sub-batches of tiles / whole matrices)
+    if (B.kpath == KPATH_LT) {     // large tiles, bf16: tcgen05 GEMMs with fused epilogues (sub-batches of tiles / whole matrices)
+      long long   n_launch = 0;
+      cudaError_t e = run_lt_path(plan->layer_dev.data(), plan->items.data() + c.begin, a.layers, a.items, c.end - c.begin,
+                                  B.T, B.Tw, mode, *hp, ws + plan->off_scratch, plan->scratch_bytes, s, &n_launch);
+      g_launches.fetch_add(n_launch);
+      if (e != cudaSuccess) return cuda_fail(e, "step: large-tile path");
+      continue;
+    }
+    if (B.kpath == KPATH_GEMM) {   // large tiles in true fp32: products go to cuBLAS (sub-batches of tiles / whole matrices)
       long long   n_launch = 0;
       cudaError_t e = run_gemm_path(plan->layer_dev.data(), plan->items.data() + c.begin, a.layers, a.items,
                                     c.end - c.begin, B.T, B.Tw, mode, B.dtype, *hp, ws + plan->off_scratch,
@@ -487,8 +497,12 @@ himuon_status himuon_phi(himuon_plan* plan, const himuon_hparams* hp, void* cuda
   return run_plan(plan, hp, MODE_PHI, cuda_stream);
 }
 
+static size_t ns_tiles_scratch_bytes() {   // fp32 cuBLAS path: one 512-tile; tcgen05 large-tile path: sub-batches of 32
+  const size_t a = gemm_path_scratch_bytes(512, 512), b = 32 * lt_path_batch_item_bytes(512, 512);
+  return a > b ? a : b;
+}
 size_t himuon_ns_tiles_workspace_bytes(void) {
-  return align_up(128 + 3 * sizeof(CUtensorMap), 256) + gemm_path_scratch_bytes(512, 512);
+  return align_up(128 + 3 * sizeof(CUtensorMap), 256) + ns_tiles_scratch_bytes();
 }
 
 himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_tiles, int32_t T,
@@ -523,6 +537,16 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
   D.w = tiles_out; D.g = const_cast<void*>(tiles_in); D.m = nullptr;
   D.ld_w = T; D.ld_g = T; D.ld_m = 0;
   D.H = (int)(n_tiles * T); D.W = T; D.tau_base = 0.f; D.dtype = dtype;
+  if (kp == KPATH_LT) {     // large tiles, bf16: tcgen05 GEMM path over the implicit list of the packed batch
+    long long   n_launch = 0;
+    cudaError_t el = cudaMemcpyAsync(ws, &D, sizeof(D), cudaMemcpyHostToDevice, s);
+    if (el != cudaSuccess) return cuda_fail(el, "ns_tiles: layer table");
+    el = run_lt_path(&D, nullptr, (const LayerDev*)ws, nullptr, n_tiles, T, T, MODE_PHI, hp,
+                     ws + align_up(128 + 3 * sizeof(CUtensorMap), 256), ns_tiles_scratch_bytes(), s, &n_launch);
+    g_launches.fetch_add(n_launch);
+    if (el != cudaSuccess) return cuda_fail(el, "ns_tiles: large-tile path");
+    return HIMUON_OK;
+  }
   if (kp == KPATH_GEMM) {   // large tiles: host walk, cuBLAS products (scratch behind the table area of the workspace)
     std::vector<WorkItem> its((size_t)n_tiles);
     for (int64_t i = 0; i < n_tiles; ++i) its[(size_t)i] = WorkItem{0, (int)i, 0, 0};

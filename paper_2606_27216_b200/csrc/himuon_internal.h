@@ -35,7 +35,7 @@ struct WorkItem {
 static_assert(sizeof(WorkItem) == 16, "WorkItem must be 16 bytes");
 
 enum Mode : int { MODE_STEP = 0, MODE_PHI = 1 };
-enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1, KPATH_WARP = 2, KPATH_GEMM = 3, KPATH_TC_FP8 = 4 };
+enum KernelPath : int { KPATH_FP32_SIMT = 0, KPATH_TC = 1, KPATH_WARP = 2, KPATH_GEMM = 3, KPATH_TC_FP8 = 4, KPATH_LT = 5 };
 inline bool kpath_uses_tma(int kp) { return kp == KPATH_TC || kp == KPATH_TC_FP8; }
 constexpr int kWholeMatrixT = 1 << 20;   // tile size of the full-matrix branch beyond the largest tile kernel (R = C = 1)
 
@@ -63,7 +63,7 @@ cudaError_t launch_tc256(const LaunchArgs& a, cudaStream_t stream);
 // kernels_warp.cu -- mma.sync bf16 path, one warp per tile, T in {16, 32}, bf16 storage.
 cudaError_t launch_warp(const LaunchArgs& a, cudaStream_t stream);
 
-// kernels_gemm.cu -- large tiles (T = 512, full-matrix branch beyond 256): cuBLAS products, host walk over the items.
+// kernels_gemm.cu -- large tiles in TRUE fp32 arithmetic (fp32 storage, HIMUON_PATH_FP32): fp32 cuBLAS products, host walk.
 size_t      gemm_path_scratch_bytes(int h, int w);        // one whole h x w block at a time
 size_t      gemm_path_batch_item_bytes(int Th, int Tw);   // per tile of a sub-batch of uniform Th x Tw tiles
 size_t      gemm_path_fixed_bytes();                      // cuBLAS workspace inside the scratch
@@ -73,6 +73,14 @@ cudaError_t run_gemm_path(const LayerDev* layers_host, const WorkItem* items_hos
                           long long* launches);
 
 // SM count of the CURRENT device (per-device cache, thread-safe).
+// kernels_lt.cu -- large tiles on bf16 storage (T = 512, full-matrix branch beyond 256, rectangular tiles): hand-written
+// persistent tcgen05 GEMMs with the Newton-Schulz step fused into their epilogues, one launch per product per sub-batch.
+size_t      lt_path_scratch_bytes(int h, int w);          // one whole h x w block
+size_t      lt_path_batch_item_bytes(int Th, int Tw);     // per tile of a sub-batch of uniform Th x Tw tiles
+cudaError_t run_lt_path(const LayerDev* layers_host, const WorkItem* items_host, const LayerDev* layers_dev,
+                        const WorkItem* items_dev, long long n_items, int T, int Tw, int mode, const himuon_hparams& hp,
+                        void* scratch, size_t scratch_bytes, cudaStream_t stream, long long* launches);
+
 int device_sm_count();
 
 // One-time kernel configuration (dynamic shared memory size) per DEVICE: `done` holds one bit per device

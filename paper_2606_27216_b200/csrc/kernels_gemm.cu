@@ -1,19 +1,19 @@
-// Large-tile path of the HiMuon hot path: tiles too big for one SM pair, i.e. T = 512 (the paper's default
-// tile size on A40) and the full-matrix branch T >= max(H, W) for matrices larger than 256
-// (the paper's T = infinity warm start).  At these sizes every product of a
-// Newton-Schulz step (Eq. 2.2) is a plain dense GEMM of library size, so the products go to
-// cuBLAS (fp32 data; TF32 tensor-core math for bf16 storage, true fp32 for fp32 storage) and only the
-// fused ends are kernels of this file:
+// Large tiles in TRUE fp32 arithmetic: fp32 storage, or HIMUON_PATH_FP32 on bf16 storage, at T >= 256 and on the
+// full-matrix branch beyond the fp32 FMA kernel's tile sizes (the <= 1e-4 path of BASELINE.json; PAPER.md:424 uses an
+// fp32 variant as its precision reference).  bf16 storage on the default path does NOT come here: its large tiles run
+// on the hand-written tcgen05 GEMM path of kernels_lt.cu.  At these sizes every product of a Newton-Schulz step
+// (Eq. 2.2) is a plain dense fp32 GEMM of library size, so the products go to cuBLAS (SGEMM,
+// CUBLAS_COMPUTE_32F) and only the fused ends are kernels of this file:
 //   k_prep   M' = beta M + G (stored), Ghat = G + beta M' | M' -> X (fp32 scratch),
 //            per-block partial sums of squares (deterministic two-stage reduction)
 //   k_scale  X <- X / (||Ghat||_F + eps), Phi_K(0) = 0
 //   K x      A = X X^T (or X^T X for tall blocks);  B = b A + c A A;  B += a I;  X <- B X (or X B)
 //   k_update W <- (1 - lr wd) W - lr tau X (Eq. 4.6; Phi mode: W <- X)
 // A tile is addressed as a strided view of the parameter's own storage (no gather); the work items of a chunk
-// are walked on the host, one tile at a time, all launches asynchronous on the caller's stream; scratch
-// (two fp32 copies of the tile, two r x r matrices, partial sums, 32 MB of cuBLAS workspace) lives in the
-// caller's workspace.  cuBLAS is bound at run time (dlopen), so the library has no link-time dependency on
-// it; if it cannot be found the large-tile path reports cudaErrorNotSupported.
+// are walked on the host, all launches asynchronous on the caller's stream; scratch (two fp32 copies of the tile, two
+// r x r matrices, partial sums, 32 MB of cuBLAS workspace) lives in the caller's workspace.  cuBLAS is bound at run
+// time (dlopen), so the library has no link-time dependency on it; if it cannot be found this path reports
+// cudaErrorNotSupported.  One handle per device, enqueueing host threads serialised by a mutex.
 #include <cublas_v2.h>
 #include <cuda_bf16.h>
 #include <dlfcn.h>
@@ -286,7 +286,7 @@ cudaError_t run_batch(const LayerDev* layers_dev, const WorkItem* items_dev, int
     if (cb.set_stream(cb.handle, s) != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
     if (cb.set_workspace(cb.handle, cws, kCublasWs) != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
   }
-  const cublasComputeType_t ct = sizeof(S) == 4 ? CUBLAS_COMPUTE_32F : CUBLAS_COMPUTE_32F_FAST_TF32;
+  const cublasComputeType_t ct = CUBLAS_COMPUTE_32F;   // this path is the true-fp32 one for either storage type
   const float one = 1.f, zero = 0.f;
   // Row-major X (h x w, ld = w) is the column-major w x h matrix Xc = X^T with leading dimension w (see run_one).
   for (int k = 0; k < hp.K; ++k) {
@@ -352,7 +352,7 @@ cudaError_t run_one(const LayerDev& L, const WorkItem& wi, int T, int mode, cons
     if (cb.set_workspace(cb.handle, cws, kCublasWs) != CUBLAS_STATUS_SUCCESS) return cudaErrorUnknown;
   }
   // fp32 storage: true fp32 products (the <= 1e-4 path); bf16 storage: TF32 tensor-core products
-  const cublasComputeType_t ct = sizeof(S) == 4 ? CUBLAS_COMPUTE_32F : CUBLAS_COMPUTE_32F_FAST_TF32;
+  const cublasComputeType_t ct = CUBLAS_COMPUTE_32F;   // this path is the true-fp32 one for either storage type
   const float one = 1.f, zero = 0.f;
   // Row-major X (h x w, ld = w) is the column-major w x h matrix Xc = X^T with leading dimension w.
   for (int k = 0; k < hp.K; ++k) {

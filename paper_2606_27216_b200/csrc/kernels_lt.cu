@@ -1,0 +1,644 @@
+// Large-tile path of the HiMuon hot path on bf16 storage: tiles that do not fit one SM pair's on-chip memory, i.e.
+// T = 512 (the paper's default tile size on A40), the full-matrix branch T >= max(H, W) beyond 256
+// (the paper's T = infinity warm start), rectangular tiles (T_h, T_w) of the tile-shape
+// study and T = 256 on widths TMA cannot store.  This is the paper's "multi-kernel path
+// with epilogue fusion" (section 4.4.1) re-designed for sm_100a: every product of a Newton-Schulz step
+// (Eq. 2.2) is ONE launch of a hand-written persistent tcgen05 GEMM over all tiles of a sub-batch,
+// with the step's elementwise work fused into its epilogue - nothing but bf16 operands, the fp32 iterate and three
+// small fp32 vectors per tile ever touches HBM between the products:
+//
+//   lt_prep    M' = beta M + G (stored); Ghat = G + beta M' | M' -> Xf (fp32) and Xb = bf16(Ghat) (scratch,
+//              tile zero-padded, stored TRANSPOSED when the tile is tall so that the Gram matrix is on the short side,
+//              PAPER.md:76); row-norm partials d_i and per-block partial sums of squares (fixed summation order).
+//              The normalisation X0 = q Ghat / (||Ghat||_F + eps), q = c^(1/4) (Phi_K(0) = 0) is NOT a
+//              pass of its own: bf16 rounding is scale-free, so the first step runs on the raw Ghat and its epilogues
+//              apply sigma = q / (||Ghat||_F + eps) (E1: sigma^2 on the accumulator and on d; E3: sigma on the result).
+//   K x  lt_gemm<E1>  ACC = Xb Xb^T;  epilogue: Ot = bf16(offdiag(ACC) + diag(d + beta/2)) -> Ob;  S_i = sum_j ACC_ij^2
+//        lt_gemm<E2>  ACC = Ot Ot^T (= B off the diagonal);  epilogue: Bb = bf16(ACC), diagonal zeroed -> Bb
+//        lt_gemm<E3>  ACC = Bb Xb;  epilogue: Xf <- (a + beta d_i + S_i) Xf + ACC;  Xb = bf16(Xf);  new d_i partials;
+//   lt_update  W <- (1 - lr wd) W - lr tau Xf / q (Eq. 4.6; Phi mode: W <- Xf / q), un-transposed
+// The numerical scheme is the one of the fused kernels (scaled state, fp32 diagonals of A and B as row scalings, the
+// operand-diagonal trick), so the accuracy is the same <= 3e-2 class.
+//
+// lt_gemm: C[b] (M x N, fp32 in TMEM) = A[b] (M x K, K-major) * B[b]; B is K-major (N x K: Gram form) or MN-major
+// (K x N: plain product).  CTA tile 128 x 256, k-block 64, 3 smem stages of 48 KB filled by TMA (3-D tensor maps over
+// the batched scratch arrays; out-of-bounds rows / columns read as zero), SS-mode tcgen05.mma 128 x 256 x 16 issued by
+// one thread, two 256-column accumulators in TMEM so that the epilogue of one tile overlaps the products of the next;
+// persistent over batch x tiles.  Warps: 0 = TMA producer of the operands, 1 = MMA issuer, 2 = TMA producer of the fp32
+// iterate's chunks (E3), 4-7 = epilogue: thread = accumulator row, and every byte of the epilogue's global traffic goes
+// through TMA (iterate chunks in, updated in place in shared memory, out; bf16 operands out) - tcgen05.ld hands a thread
+// one ROW, so direct global accesses would be 32 rows per warp instruction.
+#include <cuda_bf16.h>
+
+#include <algorithm>
+#include <cstring>
+
+#include "himuon_internal.h"
+#include "sm100_ptx.cuh"
+#include "tc_common.cuh"
+
+namespace himuon {
+namespace {
+
+using namespace ptx;
+using namespace tc;
+
+constexpr int BM = 128, BN = 256, BK = 64, kStages = 3;
+constexpr uint32_t kABytes = BM * BK * 2, kBBytes = BN * BK * 2, kStageBytes = kABytes + kBBytes;
+constexpr int kGemmThreads = 256;          // warps 0 / 1 / 2: operand producer / MMA issuer / iterate producer, 4-7 epilogue
+constexpr int kEwThreads = 256;
+constexpr int kPrepBlocks = 32;          // blocks per tile of lt_prep / lt_update (fixed: summation order)
+
+inline long long rup(long long x, long long a) { return (x + a - 1) / a * a; }
+
+// Geometry of one sub-batch: nb tiles of Th x Tw (storage orientation), iterated as rp x np with rp <= np.
+struct LtGeom {
+  int Th, Tw;            // tile extent in the parameter's storage (rows, columns)
+  int rp, np;            // iterate extent: (Th, Tw) or, transposed, (Tw, Th); multiples of 8
+  int transposed;        // 1: the iterate is the transposed tile
+  int ldx, ldr;          // leading dimensions of the [rp x np] and [rp x rp] scratch arrays (elements)
+  int ntx, ntr;          // BN-column slots of an [.. x np] / [.. x rp] array (partial-sum slots)
+  long long sx, sr;      // per-tile strides of the [rp x ldx] / [rp x ldr] arrays (elements)
+  long long sd, ss;      // per-tile strides of the d / S partial arrays (floats)
+};
+
+LtGeom make_geom(int Th, int Tw) {
+  LtGeom g;
+  g.Th = Th; g.Tw = Tw;
+  g.transposed = Th > Tw;
+  g.rp = (int)rup(std::min(Th, Tw), 8);
+  g.np = (int)rup(std::max(Th, Tw), 8);
+  g.ldx = (int)rup(g.np, 64);
+  g.ldr = (int)rup(g.rp, 64);
+  g.ntx = (g.np + BN - 1) / BN;            // partial-sum slots: one per BN-column tile of the output
+  g.ntr = (g.rp + BN - 1) / BN;
+  g.sx = (long long)g.rp * g.ldx;
+  g.sr = (long long)g.rp * g.ldr;
+  g.sd = (long long)g.ntx * g.rp;
+  g.ss = (long long)g.ntr * g.rp;
+  return g;
+}
+
+size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// Scratch of a sub-batch of nb tiles: Xf (fp32), Xb, Ob, Bb (bf16), d partials x 2 (ping-pong), S partials, ss partials.
+struct LtScratch {
+  float* xf; __nv_bfloat16 *xb, *xb2, *ob, *bb; float *d0, *d1, *sp, *ssq;   // xb / xb2: product 3 reads one, writes the other
+};
+size_t lt_item_bytes(const LtGeom& g) {
+  return a256((size_t)g.sx * 4) + 2 * a256((size_t)g.sx * 2) + 2 * a256((size_t)g.sr * 2) + 2 * a256((size_t)g.sd * 4) +
+         a256((size_t)g.ss * 4) + a256(kPrepBlocks * 4);
+}
+LtScratch carve(char* base, const LtGeom& g, int nb) {
+  LtScratch s;
+  size_t off = 0;
+  auto take = [&](size_t per) { char* p = base + off; off += (size_t)nb * per; return p; };
+  s.xf = (float*)take(a256((size_t)g.sx * 4));
+  s.xb = (__nv_bfloat16*)take(a256((size_t)g.sx * 2));
+  s.xb2 = (__nv_bfloat16*)take(a256((size_t)g.sx * 2));
+  s.ob = (__nv_bfloat16*)take(a256((size_t)g.sr * 2));
+  s.bb = (__nv_bfloat16*)take(a256((size_t)g.sr * 2));
+  s.d0 = (float*)take(a256((size_t)g.sd * 4));
+  s.d1 = (float*)take(a256((size_t)g.sd * 4));
+  s.sp = (float*)take(a256((size_t)g.ss * 4));
+  s.ssq = (float*)take(a256(kPrepBlocks * 4));
+  return s;
+}
+// per-tile strides in ELEMENTS of the carved arrays (the a256 rounding is per tile)
+long long stride_xf(const LtGeom& g) { return (long long)(a256((size_t)g.sx * 4) / 4); }
+long long stride_xb(const LtGeom& g) { return (long long)(a256((size_t)g.sx * 2) / 2); }
+long long stride_r(const LtGeom& g) { return (long long)(a256((size_t)g.sr * 2) / 2); }
+long long stride_d(const LtGeom& g) { return (long long)(a256((size_t)g.sd * 4) / 4); }
+long long stride_s(const LtGeom& g) { return (long long)(a256((size_t)g.ss * 4) / 4); }
+
+// ---- the tile of a work item -----------------------------------------------------------------------------------
+struct TileRef {
+  const __nv_bfloat16* g;
+  __nv_bfloat16* m;
+  __nv_bfloat16* w;
+  long long ld_g, ld_m, ld_w;
+  int h, w_;             // live extent (rows, columns) of this tile in the parameter
+  float tau_base;
+};
+__device__ __forceinline__ TileRef tile_ref(const LayerDev* layers, const WorkItem* items, int b, int Th, int Tw, int whole) {
+  // items == nullptr: implicit list of a packed [N, T, T] batch (himuon_ns_tiles): item i = (layer 0, r = i, c = 0);
+  // `whole` then carries the index of the sub-batch's first tile (and is never the whole-matrix flag)
+  const WorkItem wi = items ? items[b] : WorkItem{0, whole + b, 0, 0};
+  if (!items) whole = 0;
+  const LayerDev L = layers[wi.layer];
+  TileRef t;
+  const long long row0 = whole ? 0 : (long long)wi.r * Th, col0 = whole ? 0 : (long long)wi.c * Tw;
+  t.h = (int)min((long long)Th, (long long)L.H - row0);
+  t.w_ = (int)min((long long)Tw, (long long)L.W - col0);
+  t.g = reinterpret_cast<const __nv_bfloat16*>(L.g) + row0 * L.ld_g + col0;
+  t.m = L.m ? reinterpret_cast<__nv_bfloat16*>(L.m) + row0 * L.ld_m + col0 : nullptr;
+  t.w = reinterpret_cast<__nv_bfloat16*>(L.w) + row0 * L.ld_w + col0;
+  t.ld_g = L.ld_g; t.ld_m = L.ld_m; t.ld_w = L.ld_w;
+  t.tau_base = L.tau_base;
+  return t;
+}
+
+// ---- fused ends ------------------------------------------------------------------------------------------------
+// sigma = q / (||Ghat||_F + eps) of tile b from lt_prep's per-block partial sums (same order in every thread).
+__device__ __forceinline__ float tile_sigma(const float* __restrict__ ssq, int b, float eps, float qs) {
+  float tot = 0.f;
+#pragma unroll
+  for (int i = 0; i < kPrepBlocks; ++i) tot += ssq[(long long)b * kPrepBlocks + i];
+  const float nrm = sqrtf(tot);
+  return nrm > 0.f ? qs / (nrm + eps) : 0.f;          // Phi_K(0) = 0
+}
+
+// grid (kPrepBlocks, nb), one warp per row of the SCRATCH layout (rp x ldx, coalesced writes); element (i, j) of the
+// iterate is element (i, j) of the tile, or (j, i) when transposed.
+__global__ void __launch_bounds__(kEwThreads)
+lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, LtGeom g, int whole, float* __restrict__ xf,
+        long long sxf, __nv_bfloat16* __restrict__ xb, long long sxb, float* __restrict__ d0, long long sd,
+        float* __restrict__ ssq, int step_mode, float beta, int nesterov) {
+  const int b = blockIdx.y;
+  const TileRef t = tile_ref(layers, items, b, g.Th, g.Tw, whole);
+  float* X = xf + (long long)b * sxf;
+  __nv_bfloat16* Xb = xb + (long long)b * sxb;
+  float* D = d0 + (long long)b * sd;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  float ss = 0.f;
+  for (int i = blockIdx.x * (kEwThreads / 32) + warp; i < g.rp; i += kPrepBlocks * (kEwThreads / 32)) {
+    for (int slot = 0; slot < g.ntx; ++slot) {        // d partial per BN-column slot, as the E3 epilogue writes them
+      float dd = 0.f;
+      const int j1 = min((slot + 1) * BN, g.ldx);
+      for (int j = slot * BN + lane; j < j1; j += 32) {
+        const int r = g.transposed ? j : i, c = g.transposed ? i : j;    // position in the tile
+        float x = 0.f;
+        if (r < t.h && c < t.w_) {                                         // outside: B_T zero padding
+          const float gg = __bfloat162float(t.g[(long long)r * t.ld_g + c]);
+          x = gg;
+          if (step_mode) {
+            __nv_bfloat16* pm = t.m + (long long)r * t.ld_m + c;
+            const float mm = fmaf(beta, __bfloat162float(*pm), gg);
+            *pm = __float2bfloat16_rn(mm);
+            x = nesterov ? fmaf(beta, mm, gg) : mm;
+          }
+        }
+        X[(long long)i * g.ldx + j] = x;
+        Xb[(long long)i * g.ldx + j] = __float2bfloat16_rn(x);
+        dd = fmaf(x, x, dd);
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) dd += __shfl_xor_sync(0xffffffffu, dd, o);
+      if (lane == 0) D[(long long)slot * g.rp + i] = dd;
+      ss += dd;                                        // identical in every lane
+    }
+  }
+  __shared__ float red[kEwThreads / 32];
+  if (lane == 0) red[warp] = ss;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    float tot = 0.f;
+#pragma unroll
+    for (int i = 0; i < kEwThreads / 32; ++i) tot += red[i];
+    ssq[(long long)b * kPrepBlocks + blockIdx.x] = tot;
+  }
+}
+
+__global__ void __launch_bounds__(kEwThreads)
+lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, LtGeom g, int whole,
+          const float* __restrict__ xf, long long sxf, int step_mode, float keep, float lr_scale, float unq,
+          const float* __restrict__ ssq, float eps, float qs) {
+  const int b = blockIdx.y;
+  const TileRef t = tile_ref(layers, items, b, g.Th, g.Tw, whole);
+  const float* X = xf + (long long)b * sxf;
+  const float sig = ssq ? tile_sigma(ssq, b, eps, qs) : 1.f;      // K = 0: Xf still holds the raw Ghat
+  const float stepsz = (step_mode ? lr_scale * t.tau_base * unq : unq) * sig;
+  const long long n = (long long)t.h * t.w_;
+  for (long long e = (long long)blockIdx.x * kEwThreads + threadIdx.x; e < n; e += (long long)kPrepBlocks * kEwThreads) {
+    const int r = (int)(e / t.w_), c = (int)(e - (long long)r * t.w_);
+    const float x = g.transposed ? X[(long long)c * g.ldx + r] : X[(long long)r * g.ldx + c];
+    __nv_bfloat16* p = t.w + (long long)r * t.ld_w + c;
+    *p = __float2bfloat16_rn(step_mode ? fmaf(keep, __bfloat162float(*p), stepsz * x) : stepsz * x);
+  }
+}
+
+// ---- the GEMM --------------------------------------------------------------------------------------------------
+enum { EPI_GRAM = 1, EPI_B = 2, EPI_X = 3 };
+
+struct GemmParams {
+  int M, N, K;                 // C[b] is M x N; K = contraction length (all multiples of 8)
+  int nb, mt, nt;              // batch, tiles per batch item
+  const float* d_in;           // d partials of the current iterate: [b][ntx][rp]
+  float* d_out;                // E3: d partials of the new iterate
+  long long sd;
+  int ntx;
+  float* s_part;               // S partials: [b][ntr][rp]  (E1 writes, E3 reads)
+  long long ss;
+  int ntr;
+  int rp;
+  float a, beta_h;
+  int write_ops;               // E3: 0 on the last step (no operand of a next product is needed)
+  const float* ssq;            // first step only (else null): the iterate is still the raw Ghat, apply sigma here
+  float eps, qs;
+};
+
+// Epilogue staging (behind the operand stages): three 16 KB buffers.
+//   E1 / E2: one [128 rows x 64 bf16] output chunk each (128-byte swizzle, the layout of the operand tiles), rotating;
+//   E3:      buffers 0 / 1 = [128 rows x 32 fp32] chunks of the iterate (TMA in, updated in place, TMA out), buffer 2 =
+//            three [128 rows x 32 bf16] chunks of the new operand Xb (plain rows of 64 B), rotating.
+constexpr uint32_t kEpiBuf = 16384, kEpiBytes = 2 * kEpiBuf + 3 * 8192;   // 56 KB (E1 / E2 use 3 x 16 KB of it)
+struct GemmCtrl {
+  unsigned long long full[kStages], empty[kStages], tfull[2], tempty[2], xfull[2], xfree[2];
+  uint32_t tmem_base;
+};
+constexpr uint32_t kGemmSmem = kStages * kStageBytes + kEpiBytes + 1024 + 256;
+
+template <int EPI, bool B_MN>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmOut,
+        const __grid_constant__ CUtensorMap tmXf, const GemmParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t epi0 = smem0 + kStages * kStageBytes;
+  GemmCtrl* ctrl = reinterpret_cast<GemmCtrl*>(smem_raw + (smem0 - smem_u32(smem_raw)) + kStages * kStageBytes + kEpiBytes);
+  const int tid = threadIdx.x;
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const int lane = tid & 31;
+
+  if (tid == 0) {
+    for (int s = 0; s < kStages; ++s) {
+      mbar_init(smem_u32(&ctrl->full[s]), 1);
+      mbar_init(smem_u32(&ctrl->empty[s]), 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(smem_u32(&ctrl->tfull[a]), 1);
+      mbar_init(smem_u32(&ctrl->tempty[a]), 128);
+      mbar_init(smem_u32(&ctrl->xfull[a]), 1);
+      mbar_init(smem_u32(&ctrl->xfree[a]), 1);
+    }
+    fence_mbar_init();
+  }
+  if (warp == 1) tmem_alloc<512>(smem_u32(&ctrl->tmem_base));
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem_base = ctrl->tmem_base;
+
+  const long long n_tiles = (long long)p.nb * p.mt * p.nt;
+  const int kb_n = (p.K + BK - 1) / BK;
+
+  if (warp == 0) {
+    // ================= TMA producer: operands =================
+    if (elect_one()) {
+      prefetch_tmap(&tmA);
+      prefetch_tmap(&tmB);
+      int s = 0;
+      uint32_t ph = 0;
+      for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
+        const int m0 = (rem / p.nt) * BM, n0 = (rem % p.nt) * BN;
+        for (int kb = 0; kb < kb_n; ++kb) {
+          mbar_wait_parked(smem_u32(&ctrl->empty[s]), ph ^ 1);   // slot free (first pass: passes immediately)
+          const uint32_t full = smem_u32(&ctrl->full[s]);
+          const uint32_t sa = smem0 + s * kStageBytes, sbm = sa + kABytes;
+          mbar_arrive_expect_tx(full, kStageBytes);
+          tma_load_3d(sa, &tmA, kb * BK, m0, b, full);                        // A: [BM rows x 64 k]
+          if (!B_MN) {
+            tma_load_3d(sbm, &tmB, kb * BK, n0, b, full);                     // B K-major: [BN rows x 64 k]
+          } else {
+#pragma unroll
+            for (int j = 0; j < BN / 64; ++j)                                 // B MN-major: 4 x [64 k-rows x 64 n]
+              tma_load_3d(sbm + j * (BK * 128), &tmB, n0 + 64 * j, kb * BK, b, full);
+          }
+          if (++s == kStages) { s = 0; ph ^= 1; }
+        }
+      }
+    }
+    __syncwarp();
+  } else if (warp == 1) {
+    // ================= MMA issuer =================
+    if (elect_one()) {
+      const uint32_t idesc = make_idesc_bf16(BM, BN, 0, B_MN ? 1 : 0);
+      int s = 0;
+      uint32_t ph = 0;
+      uint32_t tph[2] = {0, 0};
+      int it = 0;
+      for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int ab = it & 1;
+        mbar_wait_parked(smem_u32(&ctrl->tempty[ab]), tph[ab] ^ 1);   // the epilogue has drained this accumulator
+        tph[ab] ^= 1;
+        tc_fence_after_sync();
+        const uint32_t acc = tmem_base + ab * BN;
+        for (int kb = 0; kb < kb_n; ++kb) {
+          mbar_wait_parked(smem_u32(&ctrl->full[s]), ph);
+          tc_fence_after_sync();
+          const uint32_t sa = smem0 + s * kStageBytes, sbm = sa + kABytes;
+#pragma unroll
+          for (int kk = 0; kk < BK / 16; ++kk) {
+            const uint64_t da = make_smem_desc_sw128(sa + kk * 32, 16, 1024);
+            const uint64_t db = B_MN ? make_smem_desc_sw128(sbm + kk * 2048, BK * 128, 1024)
+                                     : make_smem_desc_sw128(sbm + kk * 32, 16, 1024);
+            umma_bf16_ss(acc, da, db, idesc, (kb | kk) ? 1u : 0u);
+          }
+          umma_commit(smem_u32(&ctrl->empty[s]));                // frees the smem slot when these MMAs have read it
+          if (++s == kStages) { s = 0; ph ^= 1; }
+        }
+        umma_commit(smem_u32(&ctrl->tfull[ab]));                 // accumulator ready
+      }
+    }
+    __syncwarp();
+  } else if (warp == 2) {
+    // ================= TMA producer: chunks of the fp32 iterate for the E3 epilogue =================
+    if (EPI == EPI_X && elect_one()) {
+      prefetch_tmap(&tmXf);
+      uint32_t n = 0;                                            // running chunk counter: buffer n & 1, phase (n >> 1) & 1
+      for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
+        const int m0 = (rem / p.nt) * BM, n0 = (rem % p.nt) * BN;
+        for (int c = 0; c < BN / 32; ++c, ++n) {
+          const uint32_t buf = n & 1, par = (n >> 1) & 1;
+          mbar_wait_parked(smem_u32(&ctrl->xfree[buf]), par ^ 1);     // the chunk stored from this buffer has left it
+          const uint32_t xfull = smem_u32(&ctrl->xfull[buf]);
+          mbar_arrive_expect_tx(xfull, kEpiBuf);
+          tma_load_3d(epi0 + buf * kEpiBuf, &tmXf, n0 + 32 * c, m0, b, xfull);
+        }
+      }
+    }
+    __syncwarp();
+  } else if (warp >= 4) {
+    // ================= epilogue: thread = accumulator row (TMEM lane); all global traffic through TMA ============
+    const int wq = warp & 3;
+    const int row = wq * 32 + lane;                  // row of the tile
+    const int et = tid - 128;                        // 0..127
+    const uint32_t rsw = (uint32_t)row * 128u;       // row offset in a 128-byte-row staging buffer
+    const uint32_t sw = (uint32_t)(row & 7);         // 128-byte swizzle: 16-byte chunk c lives at c ^ (row & 7)
+    uint32_t tph[2] = {0, 0};
+    uint32_t nchunk = 0;                             // running chunk counter (E3: mirrors the producer's)
+    int it = 0;
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      const int ab = it & 1;
+      const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
+      const int mi = rem / p.nt, ni = rem % p.nt;
+      const int m0 = mi * BM, n0 = ni * BN;
+      const int i = m0 + row;                        // row of C
+      const bool row_ok = i < p.M;
+      // first step: the iterate is the raw Ghat; sigma = q / (||Ghat||_F + eps) is applied here (header)
+      const float sig = p.ssq ? tile_sigma(p.ssq, b, p.eps, p.qs) : 1.f;
+      // row scalars, fetched before the accumulator is ready (E1 needs d_i only on the diagonal tile)
+      float d_i = 0.f, s_i = 0.f;
+      const bool has_diag = row_ok && i >= n0 && i < n0 + BN;
+      if ((EPI == EPI_X && row_ok) || (EPI == EPI_GRAM && has_diag)) {
+        const float* D = p.d_in + (long long)b * p.sd;
+        for (int sl = 0; sl < p.ntx; ++sl) d_i += D[(long long)sl * p.rp + i];
+        d_i *= sig * sig;
+      }
+      if (EPI == EPI_X && row_ok) {
+        const float* S = p.s_part + (long long)b * p.ss;
+        for (int sl = 0; sl < p.ntr; ++sl) s_i += S[(long long)sl * p.rp + i];
+        s_i = p.a + fmaf(p.beta_h, d_i, s_i);        // a + B_ii, B_ii = beta d_i + (Ah^2)_ii
+      }
+      mbar_wait_parked(smem_u32(&ctrl->tfull[ab]), tph[ab]);
+      tph[ab] ^= 1;
+      tc_fence_after_sync();
+      const uint32_t acc = tmem_base + ab * BN + ((uint32_t)(wq * 32) << 16);
+      float acc_sq = 0.f;                            // E1: sum_j ACC_ij^2; E3: sum_j x_new_ij^2 over this tile's columns
+
+      if (EPI == EPI_X) {
+        const f2 s2 = pk2(s_i, s_i), g2 = pk2(sig, sig);
+        f2 sq2 = pk2(0.f, 0.f);
+#pragma unroll 1
+        for (int c = 0; c < BN / 32; ++c, ++nchunk) {
+          const uint32_t buf = nchunk & 1, par = (nchunk >> 1) & 1;
+          const uint32_t xs = epi0 + buf * kEpiBuf + rsw;                         // this row of the fp32 chunk
+          const uint32_t xbst = epi0 + 2 * kEpiBuf + (nchunk % 3) * (128 * 64) + (uint32_t)row * 64u;   // ... of the bf16 chunk
+          uint32_t r[32];
+          tmem_ld32(acc + 32 * c, r);
+          mbar_wait_parked(smem_u32(&ctrl->xfull[buf]), par);                     // the iterate's chunk has landed
+          tmem_wait_ld();
+#pragma unroll
+          for (int v = 0; v < 8; ++v) {
+            const uint32_t a = xs + (((uint32_t)v ^ sw) << 4);
+            const uint4 xv = lds128(a);
+            f2 x01 = fma2(s2, pk2u(xv.x, xv.y), pk2u(r[4 * v], r[4 * v + 1]));
+            f2 x23 = fma2(s2, pk2u(xv.z, xv.w), pk2u(r[4 * v + 2], r[4 * v + 3]));
+            x01 = mul2(x01, g2);
+            x23 = mul2(x23, g2);
+            sq2 = fma2(x01, x01, sq2);
+            sq2 = fma2(x23, x23, sq2);
+            uint32_t o0, o1, o2, o3;
+            upk2u(x01, o0, o1);
+            upk2u(x23, o2, o3);
+            sts128(a, make_uint4(o0, o1, o2, o3));                                // fp32, in place
+            r[2 * v] = cvt_bf16x2(x01);                                           // bf16 operand, packed into r[0..15]
+            r[2 * v + 1] = cvt_bf16x2(x23);
+          }
+          if (p.write_ops) {
+#pragma unroll
+            for (int v = 0; v < 4; ++v) sts128(xbst + 16 * v, make_uint4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]));
+          }
+          fence_proxy_async_smem();
+          named_bar_sync(1, 128);
+          if (et == 0) {
+            tma_store_3d(&tmXf, n0 + 32 * c, m0, b, epi0 + buf * kEpiBuf);
+            if (p.write_ops) tma_store_3d(&tmOut, n0 + 32 * c, m0, b, epi0 + 2 * kEpiBuf + (nchunk % 3) * (128 * 64));
+            tma_commit_group();
+            // all but this chunk's stores have read their buffers: the OTHER fp32 buffer may be refilled, and (through
+            // the next chunk's barrier) the bf16 buffer written two chunks ago may be rewritten
+            tma_wait_group_read1();
+            if (nchunk > 0) mbar_arrive(smem_u32(&ctrl->xfree[buf ^ 1]));
+          }
+        }
+        float q0, q1;
+        upk2(sq2, q0, q1);
+        acc_sq = q0 + q1;
+      } else {
+        const float g2s = sig * sig;
+#pragma unroll 1
+        for (int c = 0; c < BN / 64; ++c, ++nchunk) {
+          const uint32_t st = epi0 + (nchunk % 3) * kEpiBuf + rsw;                // this row of the [128 x 64] bf16 chunk
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            uint32_t r[32];
+            tmem_ld32(acc + 64 * c + 32 * hh, r);
+            tmem_wait_ld();
+            if (EPI == EPI_GRAM) {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) {
+                const float v = g2s * __uint_as_float(r[j]);
+                r[j] = __float_as_uint(v);
+                acc_sq = fmaf(v, v, acc_sq);       // columns beyond N are exact zeros (zero-filled operands)
+              }
+            }
+#pragma unroll
+            for (int v = 0; v < 4; ++v) {
+              uint4 o;
+              o.x = pack_bf16(__uint_as_float(r[8 * v + 0]), __uint_as_float(r[8 * v + 1]));
+              o.y = pack_bf16(__uint_as_float(r[8 * v + 2]), __uint_as_float(r[8 * v + 3]));
+              o.z = pack_bf16(__uint_as_float(r[8 * v + 4]), __uint_as_float(r[8 * v + 5]));
+              o.w = pack_bf16(__uint_as_float(r[8 * v + 6]), __uint_as_float(r[8 * v + 7]));
+              sts128(st + ((((uint32_t)(4 * hh + v)) ^ sw) << 4), o);
+            }
+          }
+          // the diagonal of the operand: Ot gets d_i + beta/2 (fp32, rounded once), Bb gets 0
+          const int dc = i - (n0 + 64 * c);
+          if (row_ok && dc >= 0 && dc < 64) {
+            const __nv_bfloat16 dv = __float2bfloat16_rn(EPI == EPI_GRAM ? fmaf(0.5f, p.beta_h, d_i) : 0.f);
+            const uint32_t a = st + ((((uint32_t)(dc >> 3)) ^ sw) << 4) + (uint32_t)(dc & 7) * 2u;
+            asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(*reinterpret_cast<const unsigned short*>(&dv)) : "memory");
+          }
+          fence_proxy_async_smem();
+          named_bar_sync(1, 128);
+          if (et == 0) {
+            tma_store_3d(&tmOut, n0 + 64 * c, m0, b, epi0 + (nchunk % 3) * kEpiBuf);
+            tma_commit_group();
+            tma_wait_group_read1();   // the buffer stored one chunk ago is free; the next barrier tells everyone
+          }
+        }
+      }
+      tc_fence_before_sync();
+      mbar_arrive(smem_u32(&ctrl->tempty[ab]));      // this thread has read its row of the accumulator
+      if (row_ok) {
+        if (EPI == EPI_GRAM) p.s_part[(long long)b * p.ss + (long long)ni * p.rp + i] = acc_sq;
+        else if (EPI == EPI_X) p.d_out[(long long)b * p.sd + (long long)ni * p.rp + i] = acc_sq;
+      }
+    }
+    if (et == 0) tma_wait_group0();
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc<512>(tmem_base);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* q = nullptr;
+    cudaDriverEntryPointQueryResult r;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &q, cudaEnableDefault, &r) != cudaSuccess || r != cudaDriverEntryPointSuccess)
+      q = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(q);
+  }();
+  return fn;
+}
+// [nb][rows][cols] array with row pitch ld and batch pitch sb (elements); box = box_cols x box_rows x 1.
+bool encode3d(CUtensorMap* out, void* ptr, bool fp32, int cols, int rows, int nb, long long ld, long long sb, int box_cols,
+              int box_rows, bool swizzle) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  const cuuint64_t es = fp32 ? 4 : 2;
+  cuuint64_t dims[3] = {(cuuint64_t)cols, (cuuint64_t)rows, (cuuint64_t)nb};
+  cuuint64_t strides[2] = {(cuuint64_t)ld * es, (cuuint64_t)sb * es};
+  cuuint32_t box[3] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows, 1u};
+  cuuint32_t estr[3] = {1u, 1u, 1u};
+  return fn(out, fp32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ptr, dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int EPI, bool B_MN>
+cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmOut, const CUtensorMap& tmXf,
+                        const GemmParams& p, cudaStream_t s) {
+  static DeviceOnce once;
+  cudaError_t e = configure_smem_once(once, lt_gemm<EPI, B_MN>, (int)kGemmSmem);
+  if (e != cudaSuccess) return e;
+  long long tiles = (long long)p.nb * p.mt * p.nt;
+  int grid = (int)std::min<long long>(tiles, device_sm_count());
+  if (grid < 1) return cudaSuccess;
+  lt_gemm<EPI, B_MN><<<grid, kGemmThreads, kGemmSmem, s>>>(tmA, tmB, tmOut, tmXf, p);
+  return cudaGetLastError();
+}
+
+// One sub-batch of nb tiles of geometry g.
+cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev, int nb, const LtGeom& g, int whole, int mode,
+                          const himuon_hparams& hp, char* scratch, cudaStream_t s, long long* launches) {
+  const LtScratch sc = carve(scratch, g, nb);
+  const long long sxf = stride_xf(g), sxb = stride_xb(g), sr = stride_r(g), sd = stride_d(g), ssp = stride_s(g);
+  const bool step_mode = (mode == MODE_STEP);
+  const float qs = sqrtf(sqrtf(hp.c)), beta_h = hp.b / sqrtf(hp.c);
+  const dim3 grid_t(kPrepBlocks, nb);
+  lt_prep<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xf, sxf, sc.xb, sxb, sc.d0, sd, sc.ssq,
+                                        step_mode ? 1 : 0, hp.beta, hp.nesterov);
+  *launches += 1;
+  if (hp.K > 0) {
+    // Xb is double-buffered: product 3 of a step reads Xb (all rows of a column block, as the B operand of EVERY row
+    // block's tile) while its epilogues write the new Xb, so input and output must be different arrays.
+    __nv_bfloat16* xbuf[2] = {sc.xb, sc.xb2};
+    CUtensorMap xA[2], xBk[2], xBm[2], xO[2], oA, oB, bA, xF;
+    for (int i = 0; i < 2; ++i)
+      if (!encode3d(&xA[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, BM, true) ||
+          !encode3d(&xBk[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, BN, true) ||
+          !encode3d(&xBm[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, 64, true) ||
+          !encode3d(&xO[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 32, BM, false))     // E3's 32-column output chunks
+        return cudaErrorNotSupported;
+    if (!encode3d(&oA, sc.ob, false, g.rp, g.rp, nb, g.ldr, sr, 64, BM, true) ||
+        !encode3d(&oB, sc.ob, false, g.rp, g.rp, nb, g.ldr, sr, 64, BN, true) ||
+        !encode3d(&bA, sc.bb, false, g.rp, g.rp, nb, g.ldr, sr, 64, BM, true) ||
+        !encode3d(&xF, sc.xf, true, g.np, g.rp, nb, g.ldx, sxf, 32, BM, true))               // fp32 iterate, 32-column chunks
+      return cudaErrorNotSupported;
+    GemmParams p;
+    std::memset(&p, 0, sizeof(p));
+    p.nb = nb; p.rp = g.rp; p.a = hp.a; p.beta_h = beta_h;
+    p.sd = sd; p.ntx = g.ntx; p.ss = ssp; p.ntr = g.ntr; p.s_part = sc.sp;
+    p.eps = hp.eps; p.qs = qs;
+    float* dcur = sc.d0;
+    float* dnext = sc.d1;
+    for (int k = 0; k < hp.K; ++k) {
+      const int cur = k & 1;
+      p.ssq = k == 0 ? sc.ssq : nullptr;         // first step: Xf / Xb still hold the raw Ghat
+      // A = Xb Xb^T  ->  Ot, S
+      p.M = g.rp; p.N = g.rp; p.K = g.np; p.mt = (g.rp + BM - 1) / BM; p.nt = (g.rp + BN - 1) / BN;
+      p.d_in = dcur; p.d_out = nullptr;
+      cudaError_t e = launch_gemm<EPI_GRAM, false>(xA[cur], xBk[cur], oA, xF, p, s);
+      if (e != cudaSuccess) return e;
+      // Ot Ot^T  ->  Bb
+      p.K = g.rp;
+      e = launch_gemm<EPI_B, false>(oA, oB, bA, xF, p, s);
+      if (e != cudaSuccess) return e;
+      // Bb Xb  ->  Xf, Xb, d
+      p.M = g.rp; p.N = g.np; p.K = g.rp; p.mt = (g.rp + BM - 1) / BM; p.nt = (g.np + BN - 1) / BN;
+      p.d_out = dnext; p.write_ops = (k + 1 < hp.K) ? 1 : 0;
+      e = launch_gemm<EPI_X, true>(bA, xBm[cur], xO[cur ^ 1], xF, p, s);
+      if (e != cudaSuccess) return e;
+      std::swap(dcur, dnext);
+      *launches += 3;
+    }
+  }
+  lt_update<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xf, sxf, step_mode ? 1 : 0, 1.f - hp.lr * hp.wd,
+                                          -hp.lr * hp.scale_c, 1.f / qs, hp.K == 0 ? sc.ssq : nullptr, hp.eps, qs);
+  *launches += 1;
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+size_t lt_path_batch_item_bytes(int Th, int Tw) { return lt_item_bytes(make_geom(Th, Tw)); }
+size_t lt_path_scratch_bytes(int h, int w) { return lt_item_bytes(make_geom(h, w)); }
+
+// One chunk of the work list on the large-tile path.  Uniform tiles run in sub-batches of as many tiles as the scratch
+// holds; whole-matrix items (T = kWholeMatrixT) run one at a time with the geometry of their own layer.
+cudaError_t run_lt_path(const LayerDev* layers_host, const WorkItem* items_host, const LayerDev* layers_dev,
+                        const WorkItem* items_dev, long long n_items, int T, int Tw, int mode, const himuon_hparams& hp,
+                        void* scratch, size_t scratch_bytes, cudaStream_t s, long long* launches) {
+  if (n_items < 1) return cudaSuccess;
+  if (T != kWholeMatrixT) {
+    const LtGeom g = make_geom(T, Tw);
+    const size_t per = lt_item_bytes(g);
+    if (scratch_bytes < per) return cudaErrorInvalidValue;
+    long long cap = (long long)(scratch_bytes / per);
+    if (cap > 65535) cap = 65535;     // the tile index is gridDim.y of the fused ends
+    for (long long i = 0; i < n_items; i += cap) {
+      const int nb = (int)std::min<long long>(cap, n_items - i);
+      cudaError_t e = run_sub_batch(layers_dev, items_dev ? items_dev + i : nullptr, nb, g, items_dev ? 0 : (int)i, mode, hp,
+                                    (char*)scratch, s, launches);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+  }
+  for (long long i = 0; i < n_items; ++i) {
+    const LayerDev& L = layers_host[items_host[i].layer];
+    const LtGeom g = make_geom(L.H, L.W);
+    if (scratch_bytes < lt_item_bytes(g)) return cudaErrorInvalidValue;
+    cudaError_t e = run_sub_batch(layers_dev, items_dev + i, 1, g, 1, mode, hp, (char*)scratch, s, launches);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+}  // namespace himuon

@@ -103,9 +103,9 @@ typedef struct {
 /* Hyper-parameters of Algorithm 4.1 (defaults).
  * (a,b,c) are the Newton-Schulz coefficients; scale_c is the update-scaling constant "c" of
  * sec. 4.2 (the paper uses the letter c for both). eps is ADDED to the Frobenius norm.
- * The bf16 / e4m3 tensor-core kernels (AUTO on bf16 storage at T <= 256, FP8) iterate on c^(1/4) X and need
- * c > 0: with c <= 0 (e.g. the cubic iteration (1.5, -0.5, 0)) himuon_step / himuon_phi / himuon_ns_tiles return
- * HIMUON_ERR_UNSUPPORTED before any launch; HIMUON_PATH_FP32 and the large-tile path take any finite (a, b, c). */
+ * The tcgen05 kernels (AUTO on bf16 storage at T >= 64, FP8) iterate on c^(1/4) X and need c > 0: with c <= 0
+ * (e.g. the cubic iteration (1.5, -0.5, 0)) himuon_step / himuon_phi / himuon_ns_tiles return
+ * HIMUON_ERR_UNSUPPORTED before any launch; HIMUON_PATH_FP32, fp32 storage and T = 16, 32 take any finite (a, b, c). */
 typedef struct {
   int32_t K;
   float   a, b, c;

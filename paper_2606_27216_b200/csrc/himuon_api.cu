@@ -62,10 +62,10 @@ bool valid_hparams(const himuon_hparams* hp) {
   return true;
 }
 
-// The bf16 / e4m3 tensor-core kernels (warp, tc64, tc128, tc256 and the e4m3 variants) iterate on the scaled state
-// c^(1/4) X with beta = b / sqrt(c), which needs c > 0.  The fp32 kernel and the large-tile
-// path take any finite (a, b, c), e.g. the cubic iteration (1.5, -0.5, 0).
-bool kpath_needs_positive_c(int kp) { return kp == KPATH_TC || kp == KPATH_TC_FP8 || kp == KPATH_WARP || kp == KPATH_LT; }
+// The tcgen05 kernels (tc64, tc128, tc256, their e4m3 variants and the large-tile GEMM path) iterate on the scaled state
+// c^(1/4) X with beta = b / sqrt(c), which needs c > 0.  The fp32 kernels and the warp kernel
+// (T = 16, 32: plain state, polynomial in fp32) take any finite (a, b, c), e.g. the cubic iteration (1.5, -0.5, 0).
+bool kpath_needs_positive_c(int kp) { return kp == KPATH_TC || kp == KPATH_TC_FP8 || kp == KPATH_LT; }
 bool positive_c_ok(const himuon_hparams* hp) {
   return hp->c > 0.f && std::isfinite(hp->b / std::sqrt(hp->c)) && std::isfinite(1.f / std::sqrt(std::sqrt(hp->c)));
 }

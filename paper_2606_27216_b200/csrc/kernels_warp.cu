@@ -1,38 +1,62 @@
 // Warp-level tensor-core path of the HiMuon hot path for the small tile sizes T = 16 and T = 32, bf16 storage.
 //
-// One WARP owns one T x T tile and keeps everything in registers for all K Newton-Schulz steps
-// (Eq. 2.2-2.3; nothing between the loads of G, M, W and the stores of M, W touches shared
-// or global memory).  Products use mma.sync.m16n8k16 (bf16 operands, fp32 accumulate); the
-// accumulator fragment of one product is, after rounding, the A fragment of the next (no data movement),
-// the B fragment of a Gram product X X^T is the A fragment of X itself, and the B fragment of B X is the
-// A fragment of X transposed 8 x 8 block by block with movmatrix.  These tile sizes are HBM-bound
-// (3T flop/B against a ridge of ~250), so the design goal is few instructions per element, not MMA rate.
+// One WARP owns one T x T tile and keeps the fp32 iterate in registers for all K Newton-Schulz steps
+// (Eq. 2.2-2.3; nothing between the loads of G, M, W and the stores of M, W touches global memory,
+// PAPER.md:221).  These tile sizes are HBM-bound (3T flop/B against a ridge of ~250), so the design goals are
+// (1) full-width memory transactions and a deep prefetch, (2) few instructions per element:
 //
-// Numerical scheme = the one of kernels_tc128.cu: fp32 iterate (here: accumulator-layout registers), state
-// scaled by c^(1/4) so that B = beta Ah + Ah^2 (beta = b / sqrt(c)); the O(1) diagonal of B never passes
-// through bf16 (it acts as the fp32 row scaling a + B_tt); the operand of Ah^2 carries d + beta/2 on its
-// diagonal so that offdiag(Ot Ot^T) = offdiag(B).
+//   * Column relabelling.  Phi_K(X P) = Phi_K(X) P for a permutation P, so WHICH columns of the tile a lane holds is
+//     free as long as load and store agree.  Lane (g, c) (g = lane >> 2, c = lane & 3) holds, of rows g and g + 8 of
+//     every 16-row block, the T/4 CONSECUTIVE columns c T/4 .. : one 8-byte (T = 16) or 16-byte (T = 32) access per
+//     row, a warp instruction covers whole rows, every 32-byte sector is used in full.
+//   * G, M, W of the NEXT tile stream into a warp-private shared-memory buffer with cp.async while the current
+//     tile's steps run (each lane copies exactly the bytes it reads back, so no barrier is involved).
+//   * A = X X^T and A^2 = A A^T are tf32 mma.sync.m16n8k8 products straight out of the fp32 accumulator-layout
+//     registers: with the k index relabelled (k = c <-> column 2c, k = c + 4 <-> column 2c + 1) the accumulator
+//     fragment of one product IS the A fragment and (for these X X^T-form products) the B fragment of the next, no
+//     data movement, no packing.  tf32 keeps the O(1) diagonals of A and B to 2^-11, so the polynomial
+//     B = b A + c A^2 is formed in plain fp32 and its diagonal acts as the fp32 row scaling a + B_tt - no scaled
+//     state, no operand-diagonal trick, no row-sum reductions (and any finite (a, b, c) works).
+//   * X <- (a + B_tt) X + offdiag(B) X needs X as a [k][n] operand, i.e. transposed across lanes: that product runs
+//     as bf16 mma.sync.m16n8k16 with the B fragment made by movmatrix (8 x 8 b16 transposes) from the packed iterate.
+// Measured per-tile error against the float64 oracle: see DESIGN.md section 5.
 //
-// Fragment layouts (PTX ISA, mma.m16n8k16): g = lane >> 2, c = lane & 3.
-//   accumulator of a 16 x 8 block: e = 0,1 -> (row g, col 2c + e); e = 2,3 -> (row g + 8, col 2c + e - 2)
-//   A fragment of a 16 x 16 block: a0 (row g, cols 2c..), a1 (row g+8, cols 2c..), a2 (row g, cols 8+2c..),
-//                                  a3 (row g+8, cols 8+2c..)
-//   B fragment of a 16(k) x 8(n) block: b0 (k = 2c.., n = g), b1 (k = 8+2c.., n = g)
+// Fragment layouts (PTX ISA), g = lane >> 2, c = lane & 3:
+//   accumulator of a 16 x 8 block (both shapes): e = 0,1 -> (row g, col 2c + e); e = 2,3 -> (row g + 8, col 2c + e - 2)
+//   m16n8k8 tf32:   A: a0 (g, k=c) a1 (g+8, k=c) a2 (g, k=c+4) a3 (g+8, k=c+4);   B: b0 (k=c, n=g) b1 (k=c+4, n=g)
+//   m16n8k16 bf16:  A: a0 (g, 2c..) a1 (g+8, 2c..) a2 (g, 8+2c..) a3 (g+8, 8+2c..);  B: b0 (k=2c.., n=g) b1 (k=8+2c.., n=g)
 #include <cuda_bf16.h>
+
+#include <type_traits>
 
 #include "himuon_internal.h"
 
 namespace himuon {
 namespace {
 
-constexpr int kWarpsPerBlock = 8;
-constexpr int kThreads = kWarpsPerBlock * 32;
+// T = 16: blocks of 8 warps, 4 per SM (64 registers).  T = 32: the three 32 x 32 fp32 matrices of a step (X, A, B) are 96
+// registers of a lane, so blocks of 4 warps, 3 per SM (168 registers, no spills; at 128 registers the step spills).
+template <int NB> struct Cfg {
+  static constexpr int kWarps = NB == 1 ? 8 : 4;
+  static constexpr int kBlocksPerSm = NB == 1 ? 4 : 3;
+};
 
 __device__ __forceinline__ uint32_t pack2(float lo, float hi) {
   __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<uint32_t*>(&v);
 }
-__device__ __forceinline__ void mma16816(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+__device__ __forceinline__ float bf_lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float bf_hi(uint32_t u) { return __uint_as_float(u & 0xffff0000u); }
+// fp32 -> tf32, round to nearest (ties away): the tensor core ignores the 13 low mantissa bits, so adding half of the
+// tf32 spacing to the bit pattern IS the rounding - one integer add.  (cvt.rna.tf32.f32 compiles to this add plus an
+// Inf / NaN guard, three instructions per value; the iterate and its Gram matrices are bounded by ~1.2.)
+__device__ __forceinline__ uint32_t to_tf32(float x) { return __float_as_uint(x) + 0x1000u; }
+__device__ __forceinline__ void mma_tf32(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void mma_bf16(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
   asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
                : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
                : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
@@ -42,389 +66,353 @@ __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t a) {
   asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
   return d;
 }
-__device__ __forceinline__ float quad_sum(float v) {   // sum over the 4 lanes that share a row
-  v += __shfl_xor_sync(0xffffffffu, v, 1);
-  v += __shfl_xor_sync(0xffffffffu, v, 2);
-  return v;
+template <int kBytes>
+__device__ __forceinline__ void cp_async(uint32_t dst_smem, const void* src) {
+  if constexpr (kBytes == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_smem), "l"(src) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst_smem), "l"(src) : "memory");
 }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// A 16 x 16 block of fp32 values in accumulator layout: v[nh][e], nh = column half (8 columns each).
+// A 16 x 16 block in accumulator layout: v[h][e], h = 8-column half, e as above (fp32 values or tf32 bit patterns).
 struct Blk {
   float v[2][4];
 };
-// ... rounded to bf16 as an A fragment.
-__device__ __forceinline__ void to_afrag(const Blk& x, uint32_t (&a)[4]) {
-  a[0] = pack2(x.v[0][0], x.v[0][1]);
-  a[1] = pack2(x.v[0][2], x.v[0][3]);
-  a[2] = pack2(x.v[1][0], x.v[1][1]);
-  a[3] = pack2(x.v[1][2], x.v[1][3]);
-}
-
-// ... and the bf16 rounding of what the first rounding lost (x - bf16(x)), as a second A fragment.
-__device__ __forceinline__ void to_afrag_lo(const Blk& x, const uint32_t (&hi)[4], uint32_t (&lo)[4]) {
-#pragma unroll
-  for (int r = 0; r < 4; ++r) {
-    const float a = x.v[r >> 1][2 * (r & 1)], b = x.v[r >> 1][2 * (r & 1) + 1];
-    lo[r] = pack2(a - __uint_as_float(hi[r] << 16), b - __uint_as_float(hi[r] & 0xffff0000u));
-  }
-}
-
-// Accessor of one bf16 matrix tile: element pairs (row, col), (row, col + 1) with col even relative to the
-// tile origin.  `fast` = base pointer 4-byte aligned, ld even and the tile origin column even (always: T is
-// even), so a pair is one 32-bit access; otherwise two 16-bit accesses.  Out-of-range elements read as zero
-// (= the zero padding of B_T) and are not written (= the crop of B_T^-1).
-struct TileIO {
-  __nv_bfloat16* p;
-  long long ld;
-  int H, W;      // extent of the matrix
-  bool fast;
-  __device__ __forceinline__ void load2(int row, int col, float& lo, float& hi) const {
-    lo = hi = 0.f;
-    if (row >= H || col >= W) return;
-    const __nv_bfloat16* q = p + (long long)row * ld + col;
-    if (fast && col + 1 < W) {
-      const uint32_t u = *reinterpret_cast<const uint32_t*>(q);
-      lo = __uint_as_float(u << 16);
-      hi = __uint_as_float(u & 0xffff0000u);
-    } else {
-      lo = __bfloat162float(q[0]);
-      if (col + 1 < W) hi = __bfloat162float(q[1]);
-    }
-  }
-  // the same pair as stored bits (lo in the low half), zero outside the matrix
-  __device__ __forceinline__ uint32_t load2_raw(int row, int col) const {
-    if (row >= H || col >= W) return 0u;
-    const __nv_bfloat16* q = p + (long long)row * ld + col;
-    if (fast && col + 1 < W) return __ldg(reinterpret_cast<const uint32_t*>(q));
-    uint32_t u = *reinterpret_cast<const unsigned short*>(q);
-    if (col + 1 < W) u |= (uint32_t)(*reinterpret_cast<const unsigned short*>(q + 1)) << 16;
-    return u;
-  }
-  __device__ __forceinline__ void store2(int row, int col, float lo, float hi) const {
-    if (row >= H || col >= W) return;
-    __nv_bfloat16* q = p + (long long)row * ld + col;
-    if (fast && col + 1 < W) {
-      *reinterpret_cast<uint32_t*>(q) = pack2(lo, hi);
-    } else {
-      q[0] = __float2bfloat16_rn(lo);
-      if (col + 1 < W) q[1] = __float2bfloat16_rn(hi);
-    }
-  }
+struct BlkU {
+  uint32_t v[2][4];
 };
-__device__ __forceinline__ TileIO make_io(void* ptr, long long ld, int H, int W) {
-  TileIO io;
-  io.p = reinterpret_cast<__nv_bfloat16*>(ptr);
-  io.ld = ld;
-  io.H = H;
-  io.W = W;
-  io.fast = ((reinterpret_cast<uintptr_t>(ptr) & 3) == 0) && ((ld & 1) == 0);
-  return io;
-}
 
-// Interior tile with 32-bit-aligned rows: every element pair of the thread is one unchecked 32-bit access at
-// base + (2 i + rr) * rows8 + (2 j + nh) * 4 words (base = the thread's first pair, rows8 = 8 rows in words).
-struct FastTile {
-  bool ok;
-  long long g8, m8, w8;         // 8 rows of G / M / W in 32-bit words
-  const uint32_t* g;
-  uint32_t* m;
-  uint32_t* w;
-};
-__device__ __forceinline__ FastTile make_fast(const LayerDev& L, int row0, int col0, int T, int g, int c, bool step_mode) {
-  FastTile f;
-  const uintptr_t al = reinterpret_cast<uintptr_t>(L.g) | reinterpret_cast<uintptr_t>(L.w) |
-                       (step_mode ? reinterpret_cast<uintptr_t>(L.m) : 0);
-  f.ok = (row0 + T <= L.H) && (col0 + T <= L.W) && ((al & 3) == 0) && (((L.ld_g | L.ld_w | (step_mode ? L.ld_m : 0)) & 1) == 0);
-  const long long r = row0 + g, cc = col0 + 2 * c;
-  f.g = reinterpret_cast<const uint32_t*>(reinterpret_cast<const __nv_bfloat16*>(L.g) + r * L.ld_g + cc);
-  f.m = reinterpret_cast<uint32_t*>(reinterpret_cast<__nv_bfloat16*>(L.m) + r * L.ld_m + cc);
-  f.w = reinterpret_cast<uint32_t*>(reinterpret_cast<__nv_bfloat16*>(L.w) + r * L.ld_w + cc);
-  f.g8 = 4 * L.ld_g;
-  f.m8 = 4 * L.ld_m;
-  f.w8 = 4 * L.ld_w;
-  return f;
-}
-
-// The K Newton-Schulz steps on one tile held in registers.  SPLIT: the bf16 operand made from the fp32
-// iterate is complemented by the bf16 rounding of its remainder (Gram product with 3 MMAs, B X with 2).
-template <int NB, bool SPLIT>
-__device__ __forceinline__ void ns_steps(Blk (&x)[NB][NB], float (&d)[NB][2], const himuon_hparams& hp, float beta_h,
-                                         bool pd0, bool pd1) {
-#pragma unroll 1
-  for (int k = 0; k < hp.K; ++k) {
-    uint32_t xa[NB][NB][4], xl[SPLIT ? NB : 1][SPLIT ? NB : 1][4];
+// D (+)= P Q^T for 16 x 16 blocks held in accumulator layout (tf32 bit patterns): k-slice (kh) of P as the A fragment,
+// rows 8 nn + g of Q as the B fragment - all operands are the lane's own registers.
+__device__ __forceinline__ void gram_block(Blk& d, const BlkU& p, const BlkU& q) {
 #pragma unroll
-    for (int i = 0; i < NB; ++i)
+  for (int nn = 0; nn < 2; ++nn)
 #pragma unroll
-      for (int j = 0; j < NB; ++j) {
-        to_afrag(x[i][j], xa[i][j]);
-        if (SPLIT) to_afrag_lo(x[i][j], xa[i][j], xl[SPLIT ? i : 0][SPLIT ? j : 0]);
-      }
-
-    // Ah = Xb Xb^T
-    Blk A[NB][NB];
-#pragma unroll
-    for (int i = 0; i < NB; ++i)
-#pragma unroll
-      for (int j = 0; j < NB; ++j)
-#pragma unroll
-        for (int nh = 0; nh < 2; ++nh) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) A[i][j].v[nh][e] = 0.f;
-#pragma unroll
-          for (int kb = 0; kb < NB; ++kb) {
-            mma16816(A[i][j].v[nh], xa[i][kb], xa[j][kb][nh], xa[j][kb][nh + 2]);
-            if (SPLIT) {   // (Xh + Xl)(Xh + Xl)^T without the Xl Xl^T term
-              mma16816(A[i][j].v[nh], xa[i][kb], xl[SPLIT ? j : 0][SPLIT ? kb : 0][nh], xl[SPLIT ? j : 0][SPLIT ? kb : 0][nh + 2]);
-              mma16816(A[i][j].v[nh], xl[SPLIT ? i : 0][SPLIT ? kb : 0], xa[j][kb][nh], xa[j][kb][nh + 2]);
-            }
-          }
-        }
-    // a + B_tt with B_tt = beta d_t + (Ah^2)_tt, (Ah^2)_tt = sum_j Ah_tj^2: fp32 row scaling
-    float si[NB][2];
-#pragma unroll
-    for (int i = 0; i < NB; ++i) {
-      float p0 = 0.f, p1 = 0.f;
-#pragma unroll
-      for (int j = 0; j < NB; ++j)
-#pragma unroll
-        for (int nh = 0; nh < 2; ++nh) {
-          p0 = fmaf(A[i][j].v[nh][0], A[i][j].v[nh][0], fmaf(A[i][j].v[nh][1], A[i][j].v[nh][1], p0));
-          p1 = fmaf(A[i][j].v[nh][2], A[i][j].v[nh][2], fmaf(A[i][j].v[nh][3], A[i][j].v[nh][3], p1));
-        }
-      si[i][0] = hp.a + fmaf(beta_h, d[i][0], quad_sum(p0));
-      si[i][1] = hp.a + fmaf(beta_h, d[i][1], quad_sum(p1));
-      // Ot = offdiag(Ah) + diag(d + beta/2): offdiag(Ot Ot^T) = offdiag(beta Ah + Ah^2)
-      const float dv0 = fmaf(0.5f, beta_h, d[i][0]), dv1 = fmaf(0.5f, beta_h, d[i][1]);
-      if (pd0) { A[i][i].v[0][0] = dv0; A[i][i].v[1][2] = dv1; }
-      if (pd1) { A[i][i].v[0][1] = dv0; A[i][i].v[1][3] = dv1; }
-    }
-    uint32_t oa[NB][NB][4];
-#pragma unroll
-    for (int i = 0; i < NB; ++i)
-#pragma unroll
-      for (int j = 0; j < NB; ++j) to_afrag(A[i][j], oa[i][j]);
-
-    // B (off the diagonal) = Ot Ot^T, rounded to bf16 with the diagonal zeroed
-    uint32_t ba[NB][NB][4];
-#pragma unroll
-    for (int i = 0; i < NB; ++i)
-#pragma unroll
-      for (int j = 0; j < NB; ++j) {
-        Blk Bm;
-#pragma unroll
-        for (int nh = 0; nh < 2; ++nh) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) Bm.v[nh][e] = 0.f;
-#pragma unroll
-          for (int kb = 0; kb < NB; ++kb) mma16816(Bm.v[nh], oa[i][kb], oa[j][kb][nh], oa[j][kb][nh + 2]);
-        }
-        if (i == j) {
-          if (pd0) { Bm.v[0][0] = 0.f; Bm.v[1][2] = 0.f; }
-          if (pd1) { Bm.v[0][1] = 0.f; Bm.v[1][3] = 0.f; }
-        }
-        to_afrag(Bm, ba[i][j]);
-      }
-
-    // Xh <- (a + B_tt) Xh + offdiag(B) Xb: scale the state, then accumulate the product onto it
-#pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      uint32_t xt[NB][2][2], xtl[SPLIT ? NB : 1][2][2];   // B fragments of Xb(kb, j): [kb][nh][b0 / b1]
-#pragma unroll
-      for (int kb = 0; kb < NB; ++kb) {
-        xt[kb][0][0] = movmatrix_trans(xa[kb][j][0]);
-        xt[kb][0][1] = movmatrix_trans(xa[kb][j][1]);
-        xt[kb][1][0] = movmatrix_trans(xa[kb][j][2]);
-        xt[kb][1][1] = movmatrix_trans(xa[kb][j][3]);
-        if (SPLIT) {
-          xtl[SPLIT ? kb : 0][0][0] = movmatrix_trans(xl[SPLIT ? kb : 0][SPLIT ? j : 0][0]);
-          xtl[SPLIT ? kb : 0][0][1] = movmatrix_trans(xl[SPLIT ? kb : 0][SPLIT ? j : 0][1]);
-          xtl[SPLIT ? kb : 0][1][0] = movmatrix_trans(xl[SPLIT ? kb : 0][SPLIT ? j : 0][2]);
-          xtl[SPLIT ? kb : 0][1][1] = movmatrix_trans(xl[SPLIT ? kb : 0][SPLIT ? j : 0][3]);
-        }
-      }
-#pragma unroll
-      for (int i = 0; i < NB; ++i)
-#pragma unroll
-        for (int nh = 0; nh < 2; ++nh) {
-          x[i][j].v[nh][0] *= si[i][0];
-          x[i][j].v[nh][1] *= si[i][0];
-          x[i][j].v[nh][2] *= si[i][1];
-          x[i][j].v[nh][3] *= si[i][1];
-#pragma unroll
-          for (int kb = 0; kb < NB; ++kb) {
-            mma16816(x[i][j].v[nh], ba[i][kb], xt[kb][nh][0], xt[kb][nh][1]);
-            if (SPLIT) mma16816(x[i][j].v[nh], ba[i][kb], xtl[SPLIT ? kb : 0][nh][0], xtl[SPLIT ? kb : 0][nh][1]);
-          }
-        }
-    }
-    if (k + 1 < hp.K) {
-#pragma unroll
-      for (int i = 0; i < NB; ++i) {
-        float p0 = 0.f, p1 = 0.f;
-#pragma unroll
-        for (int j = 0; j < NB; ++j)
-#pragma unroll
-          for (int nh = 0; nh < 2; ++nh) {
-            p0 = fmaf(x[i][j].v[nh][0], x[i][j].v[nh][0], fmaf(x[i][j].v[nh][1], x[i][j].v[nh][1], p0));
-            p1 = fmaf(x[i][j].v[nh][2], x[i][j].v[nh][2], fmaf(x[i][j].v[nh][3], x[i][j].v[nh][3], p1));
-          }
-        d[i][0] = quad_sum(p0);
-        d[i][1] = quad_sum(p1);
-      }
-    }
-  }
+    for (int kh = 0; kh < 2; ++kh)
+      mma_tf32(d.v[nn], p.v[kh][0], p.v[kh][2], p.v[kh][1], p.v[kh][3], q.v[kh][2 * nn], q.v[kh][2 * nn + 1]);
 }
 
 template <int NB>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(Cfg<NB>::kWarps * 32, Cfg<NB>::kBlocksPerSm)
 himuon_warp_kernel(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, long long n_items,
                    int mode, himuon_hparams hp) {
   constexpr int T = 16 * NB;
-  const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3;
+  constexpr int kWarpsPerBlock = Cfg<NB>::kWarps;
+  constexpr int kLaneBytes = T / 2;                // bytes of a row held by one lane: 8 (T = 16) / 16 (T = 32)
+  constexpr int kRowBytes = 2 * T;
+  constexpr int kTileBytes = T * kRowBytes;
+  constexpr int kRowsPerLane = 2 * NB;             // rows 16 i + g and 16 i + g + 8
+  typedef typename std::conditional<NB == 1, uint2, uint4>::type vec_t;   // one lane's share of a row
+  extern __shared__ __align__(16) uint8_t smem[];
+  const int lane = threadIdx.x & 31, g = lane >> 2, c = lane & 3, warp = threadIdx.x >> 5;
   const bool step_mode = (mode == MODE_STEP);
   // the diagonal element of row g (and of row g + 8) of a diagonal 16 x 16 block sits in lane c == g >> 1,
   // accumulator slot e = g & 1 of column half 0 (slot 2 + (g & 1) of column half 1)
-  const bool pd0 = (c == (g >> 1)) && !(g & 1), pd1 = (c == (g >> 1)) && (g & 1);
-  const float qs = sqrtf(sqrtf(hp.c));          // state Xh = c^(1/4) X, see kernels_tc128.cu
-  const float beta_h = hp.b / sqrtf(hp.c);
+  const bool pd = (c == (g >> 1));
+  const int pe = g & 1;
+  const int diag_src = (lane & ~3) | (g >> 1);
   const long long stride = (long long)gridDim.x * kWarpsPerBlock;
+  // warp-private staging: 2 buffers x (G, M, W); a lane's bytes of row r: r * kRowBytes + c * kLaneBytes
+  const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem) + warp * (2 * 3 * kTileBytes);
+  const uint32_t lane_off = (uint32_t)g * kRowBytes + (uint32_t)c * kLaneBytes;
 
-  // Software pipeline over the warp's tiles: the work item, the layer descriptor and the raw G / M bits of
-  // the NEXT tile are requested before the Newton-Schulz steps of the current one, and W of the current
-  // tile before its steps, so that the dependent chain item -> layer -> data never stalls the warp.
-  auto fetch = [&](long long i, LayerDev& L, int& row0, int& col0, uint32_t (&gq)[NB * NB * 4], uint32_t (&mq)[NB * NB * 4]) {
+  struct TileAt {
+    const uint8_t *pg;
+    uint8_t *pm, *pw;         // this lane's first element (row g of the tile, its column group)
+    long long sg, sm, sw;     // row strides in bytes
+    int rows, cols;           // live extent of the tile
+    float tau_base;
+    bool fast;                // interior tile, aligned: vector accesses without bounds checks
+  };
+  auto locate = [&](long long i) {
     WorkItem wi;
     if (items) wi = items[i];
     else { wi.layer = 0; wi.r = (int)i; wi.c = 0; wi.pad = 0; }
-    L = layers[wi.layer];
-    row0 = wi.r * T;
-    col0 = wi.c * T;
-    const FastTile ft = make_fast(L, row0, col0, T, g, c, step_mode);
-    if (ft.ok) {
+    const LayerDev L = layers[wi.layer];
+    TileAt t;
+    const long long row0 = (long long)wi.r * T, col0 = (long long)wi.c * T;
+    t.rows = (int)min((long long)T, L.H - row0);
+    t.cols = (int)min((long long)T, L.W - col0);
+    t.sg = L.ld_g * 2; t.sm = L.ld_m * 2; t.sw = L.ld_w * 2;
+    const long long col = col0 + c * (T / 4);
+    t.pg = reinterpret_cast<const uint8_t*>(L.g) + (row0 + g) * t.sg + col * 2;
+    t.pm = L.m ? reinterpret_cast<uint8_t*>(L.m) + (row0 + g) * t.sm + col * 2 : nullptr;
+    t.pw = reinterpret_cast<uint8_t*>(L.w) + (row0 + g) * t.sw + col * 2;
+    const uintptr_t al = reinterpret_cast<uintptr_t>(L.g) | reinterpret_cast<uintptr_t>(L.w) | (uintptr_t)t.sg | (uintptr_t)t.sw |
+                         (step_mode ? (reinterpret_cast<uintptr_t>(L.m) | (uintptr_t)t.sm) : 0);
+    t.fast = (t.rows == T) && (t.cols == T) && ((al & (kLaneBytes - 1)) == 0);
+    t.tau_base = L.tau_base;
+    return t;
+  };
+  // stream a tile's G, M (and W) into staging buffer `buf` (fast tiles only; others are read directly when needed)
+  auto prefetch = [&](const TileAt& t, int buf) {
+    if (!t.fast) return;
+    const uint32_t dst = sbase + buf * (3 * kTileBytes) + lane_off;
 #pragma unroll
-      for (int q = 0; q < NB * NB * 4; ++q) {
-        const int i2 = q / (NB * 4), j2 = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
-        gq[q] = __ldg(ft.g + (2 * i2 + rr) * ft.g8 + (2 * j2 + nh) * 4);
-        mq[q] = step_mode ? ft.m[(2 * i2 + rr) * ft.m8 + (2 * j2 + nh) * 4] : 0u;
+    for (int r = 0; r < kRowsPerLane; ++r) {
+      cp_async<kLaneBytes>(dst + r * 8 * kRowBytes, t.pg + (long long)r * 8 * t.sg);
+      if (step_mode) {
+        cp_async<kLaneBytes>(dst + kTileBytes + r * 8 * kRowBytes, t.pm + (long long)r * 8 * t.sm);
+        cp_async<kLaneBytes>(dst + 2 * kTileBytes + r * 8 * kRowBytes, t.pw + (long long)r * 8 * t.sw);
       }
-      return;
-    }
-    const TileIO ioG = make_io(L.g, L.ld_g, L.H, L.W);
-    const TileIO ioM = make_io(L.m, L.ld_m, L.H, L.W);
-#pragma unroll
-    for (int q = 0; q < NB * NB * 4; ++q) {
-      const int i2 = q / (NB * 4), j2 = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
-      const int row = row0 + 16 * i2 + g + 8 * rr, col = col0 + 16 * j2 + 8 * nh + 2 * c;
-      gq[q] = ioG.load2_raw(row, col);
-      mq[q] = step_mode ? ioM.load2_raw(row, col) : 0u;
     }
   };
+  // one lane's share of row r (0 .. 2 NB - 1 -> tile row g + 8 r) of a tensor: staging buffer (fast) or global memory
+  auto read_row = [&](const TileAt& t, int buf, int which, const uint8_t* gp, long long gs, int r, uint32_t (&w)[kLaneBytes / 4]) {
+    if (t.fast) {
+      const uint32_t a = sbase + buf * (3 * kTileBytes) + which * kTileBytes + lane_off + r * 8 * kRowBytes;
+      if constexpr (NB == 1) asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(w[0]), "=r"(w[1]) : "r"(a));
+      else asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(a));
+    } else {   // edge or unaligned tile: element by element, zero outside the matrix (B_T padding)
+      const unsigned short* p = reinterpret_cast<const unsigned short*>(gp + (long long)r * 8 * gs);
+      const int row = g + 8 * r;
+#pragma unroll
+      for (int q = 0; q < kLaneBytes / 4; ++q) {
+        const int col = c * (T / 4) + 2 * q;
+        uint32_t lo = 0, hi = 0;
+        if (gp && row < t.rows) {
+          if (col < t.cols) lo = p[2 * q];
+          if (col + 1 < t.cols) hi = p[2 * q + 1];
+        }
+        w[q] = lo | (hi << 16);
+      }
+    }
+  };
+  auto write_row = [&](const TileAt& t, uint8_t* gp, long long gs, int r, const uint32_t (&w)[kLaneBytes / 4]) {
+    if (t.fast) {
+      vec_t v;
+      if constexpr (NB == 1) v = make_uint2(w[0], w[1]);
+      else v = make_uint4(w[0], w[1], w[2], w[3]);
+      *reinterpret_cast<vec_t*>(gp + (long long)r * 8 * gs) = v;
+    } else {   // crop of B_T^-1
+      unsigned short* p = reinterpret_cast<unsigned short*>(gp + (long long)r * 8 * gs);
+      const int row = g + 8 * r;
+#pragma unroll
+      for (int q = 0; q < kLaneBytes / 4; ++q) {
+        const int col = c * (T / 4) + 2 * q;
+        if (row < t.rows) {
+          if (col < t.cols) p[2 * q] = (unsigned short)(w[q] & 0xffffu);
+          if (col + 1 < t.cols) p[2 * q + 1] = (unsigned short)(w[q] >> 16);
+        }
+      }
+    }
+  };
+  // Register home of a lane's 4 consecutive columns of 16-column block j, rows g (rr = 0) / g + 8 (rr = 1) of block row i:
+  // x[i][j].v[0][2 rr + {0,1}], x[i][j].v[1][2 rr + {0,1}].  Word q of the lane's row share = columns 2q, 2q + 1 of its
+  // group: block j = q / 2, half h = q % 2.
 
-  long long it = (long long)blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
-  LayerDev Ln;
-  int rown = 0, coln = 0;
-  uint32_t gq[NB * NB * 4], mq[NB * NB * 4];
-  if (it < n_items) fetch(it, Ln, rown, coln, gq, mq);
+  long long it = (long long)blockIdx.x * kWarpsPerBlock + warp;
+  TileAt cur;
+  int buf = 0;
+  if (it < n_items) {
+    cur = locate(it);
+    prefetch(cur, 0);
+  }
+  cp_async_commit();
 
   while (it < n_items) {
-    const LayerDev L = Ln;
-    const int row0 = rown, col0 = coln;
-    const TileIO ioM = make_io(L.m, L.ld_m, L.H, L.W);
-    const TileIO ioW = make_io(L.w, L.ld_w, L.H, L.W);
-    const FastTile ft = make_fast(L, row0, col0, T, g, c, step_mode);
+    const long long nx = it + stride;
+    TileAt nxt = cur;
+    cp_async_wait_all();                 // this tile's G, M, W are in the staging buffer
+    if (nx < n_items) {
+      nxt = locate(nx);
+      prefetch(nxt, buf ^ 1);            // in flight during this tile's steps
+    }
+    cp_async_commit();
 
     // ---------------- P: momentum, Frobenius normalisation ----------
     Blk x[NB][NB];
     float ss = 0.f;
 #pragma unroll
-    for (int q = 0; q < NB * NB * 4; ++q) {
-      const int i = q / (NB * 4), j = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
-      const int row = row0 + 16 * i + g + 8 * rr, col = col0 + 16 * j + 8 * nh + 2 * c;
-      const float g0 = __uint_as_float(gq[q] << 16), g1 = __uint_as_float(gq[q] & 0xffff0000u);
-      float h0 = g0, h1 = g1;
-      if (step_mode) {
-        const float m0 = fmaf(hp.beta, __uint_as_float(mq[q] << 16), g0);
-        const float m1 = fmaf(hp.beta, __uint_as_float(mq[q] & 0xffff0000u), g1);
-        if (ft.ok) ft.m[(2 * i + rr) * ft.m8 + (2 * j + nh) * 4] = pack2(m0, m1);
-        else ioM.store2(row, col, m0, m1);
-        h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;     // Ghat = G + beta M' (Nesterov) | M'
-        h1 = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
+    for (int r = 0; r < kRowsPerLane; ++r) {
+      const int i = r >> 1, rr = r & 1;
+      uint32_t gw[kLaneBytes / 4], mw[kLaneBytes / 4], mo[kLaneBytes / 4];
+      read_row(cur, buf, 0, cur.pg, cur.sg, r, gw);
+      if (step_mode) read_row(cur, buf, 1, cur.pm, cur.sm, r, mw);
+#pragma unroll
+      for (int q = 0; q < kLaneBytes / 4; ++q) {
+        const float g0 = bf_lo(gw[q]), g1 = bf_hi(gw[q]);
+        float h0 = g0, h1 = g1;
+        if (step_mode) {
+          const float m0 = fmaf(hp.beta, bf_lo(mw[q]), g0), m1 = fmaf(hp.beta, bf_hi(mw[q]), g1);
+          mo[q] = pack2(m0, m1);
+          h0 = hp.nesterov ? fmaf(hp.beta, m0, g0) : m0;     // Ghat = G + beta M' (Nesterov) | M'
+          h1 = hp.nesterov ? fmaf(hp.beta, m1, g1) : m1;
+        }
+        x[i][q >> 1].v[q & 1][2 * rr] = h0;
+        x[i][q >> 1].v[q & 1][2 * rr + 1] = h1;
+        ss = fmaf(h0, h0, fmaf(h1, h1, ss));
       }
-      x[i][j].v[nh][2 * rr] = h0;
-      x[i][j].v[nh][2 * rr + 1] = h1;
-      ss = fmaf(h0, h0, fmaf(h1, h1, ss));
+      if (step_mode) write_row(cur, cur.pm, cur.sm, r, mo);
     }
-    const long long nx = it + stride;
-    if (nx < n_items) fetch(nx, Ln, rown, coln, gq, mq);      // consumed in the next iteration
-    uint32_t wq[NB * NB * 4];                                  // W of this tile, consumed after the steps
 #pragma unroll
-    for (int q = 0; q < NB * NB * 4; ++q) {
-      const int i = q / (NB * 4), j = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
-      if (!step_mode) wq[q] = 0u;
-      else if (ft.ok) wq[q] = ft.w[(2 * i + rr) * ft.w8 + (2 * j + nh) * 4];
-      else wq[q] = ioW.load2_raw(row0 + 16 * i + g + 8 * rr, col0 + 16 * j + 8 * nh + 2 * c);
-    }
-    float tot = ss;
+    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    const float nrm = sqrtf(ss);
+    const float inv = nrm > 0.f ? 1.f / (nrm + hp.eps) : 0.f;   // Phi_K(0) = 0
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-    const float nrm = sqrtf(tot);
-    const float inv = nrm > 0.f ? qs / (nrm + hp.eps) : 0.f;   // Phi_K(0) = 0
-    float d[NB][2];                                             // d = diag(Ah) in fp32, rows g / g + 8 of block row i
-#pragma unroll
-    for (int i = 0; i < NB; ++i) {
-      float p0 = 0.f, p1 = 0.f;
+    for (int i = 0; i < NB; ++i)
 #pragma unroll
       for (int j = 0; j < NB; ++j)
 #pragma unroll
-        for (int nh = 0; nh < 2; ++nh)
+        for (int h = 0; h < 2; ++h)
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float v = x[i][j].v[nh][e] * inv;
-            x[i][j].v[nh][e] = v;
-            if (e < 2) p0 = fmaf(v, v, p0); else p1 = fmaf(v, v, p1);
-          }
-      d[i][0] = quad_sum(p0);
-      d[i][1] = quad_sum(p1);
-    }
+          for (int e = 0; e < 4; ++e) x[i][j].v[h][e] *= inv;
 
     // ---------------- K Newton-Schulz steps -------------------------------------------
-    // Ragged edge tiles have few rows or columns and so few singular directions to average rounding errors
-    // over; they run with the iterate split into bf16 hi + lo parts (errors ~4x smaller, 2x the MMAs).
-    const bool ragged = (row0 + T > L.H) || (col0 + T > L.W);
-    if (ragged) ns_steps<NB, true>(x, d, hp, beta_h, pd0, pd1);
-    else ns_steps<NB, false>(x, d, hp, beta_h, pd0, pd1);
+#pragma unroll 1
+    for (int k = 0; k < hp.K; ++k) {
+      // A = X X^T (tf32)
+      Blk A[NB][NB];
+      {
+        BlkU xt[NB][NB];
+#pragma unroll
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+          for (int j = 0; j < NB; ++j)
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) xt[i][j].v[h][e] = to_tf32(x[i][j].v[h][e]);
+#pragma unroll
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+          for (int j = 0; j < NB; ++j) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) A[i][j].v[h][e] = 0.f;
+#pragma unroll
+            for (int kb = 0; kb < NB; ++kb) gram_block(A[i][j], xt[i][kb], xt[j][kb]);
+          }
+      }
+      // B = b A + c A^2 (A symmetric: A^2 = A A^T, the same register-only product form)
+      Blk Bm[NB][NB];
+      {
+        BlkU at[NB][NB];
+#pragma unroll
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+          for (int j = 0; j < NB; ++j)
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) at[i][j].v[h][e] = to_tf32(A[i][j].v[h][e]);
+#pragma unroll
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+          for (int j = 0; j < NB; ++j) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) Bm[i][j].v[h][e] = 0.f;
+#pragma unroll
+            for (int kb = 0; kb < NB; ++kb) gram_block(Bm[i][j], at[i][kb], at[j][kb]);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) Bm[i][j].v[h][e] = fmaf(hp.c, Bm[i][j].v[h][e], hp.b * A[i][j].v[h][e]);
+          }
+      }
+      // a + B_tt as an fp32 row scaling; the diagonal leaves the bf16 operand
+      float s0[NB], s1[NB];
+#pragma unroll
+      for (int i = 0; i < NB; ++i) {
+        const float d0 = pe ? Bm[i][i].v[0][1] : Bm[i][i].v[0][0];      // (g, g) where this lane holds it
+        const float d1 = pe ? Bm[i][i].v[1][3] : Bm[i][i].v[1][2];      // (g + 8, g + 8)
+        s0[i] = hp.a + __shfl_sync(0xffffffffu, d0, diag_src);
+        s1[i] = hp.a + __shfl_sync(0xffffffffu, d1, diag_src);
+        if (pd) {
+          if (pe) { Bm[i][i].v[0][1] = 0.f; Bm[i][i].v[1][3] = 0.f; }
+          else { Bm[i][i].v[0][0] = 0.f; Bm[i][i].v[1][2] = 0.f; }
+        }
+      }
+      // X <- (a + B_tt) X + offdiag(B) Xb   (bf16 m16n8k16; B fragment of Xb by movmatrix)
+      uint32_t ba[NB][NB][4], xa[NB][NB][4];
+#pragma unroll
+      for (int i = 0; i < NB; ++i)
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+          ba[i][j][0] = pack2(Bm[i][j].v[0][0], Bm[i][j].v[0][1]);
+          ba[i][j][1] = pack2(Bm[i][j].v[0][2], Bm[i][j].v[0][3]);
+          ba[i][j][2] = pack2(Bm[i][j].v[1][0], Bm[i][j].v[1][1]);
+          ba[i][j][3] = pack2(Bm[i][j].v[1][2], Bm[i][j].v[1][3]);
+          xa[i][j][0] = pack2(x[i][j].v[0][0], x[i][j].v[0][1]);
+          xa[i][j][1] = pack2(x[i][j].v[0][2], x[i][j].v[0][3]);
+          xa[i][j][2] = pack2(x[i][j].v[1][0], x[i][j].v[1][1]);
+          xa[i][j][3] = pack2(x[i][j].v[1][2], x[i][j].v[1][3]);
+        }
+#pragma unroll
+      for (int j = 0; j < NB; ++j) {
+        uint32_t xb[NB][2][2];   // B fragments of Xb(kb, j): [kb][h][b0 / b1]
+#pragma unroll
+        for (int kb = 0; kb < NB; ++kb) {
+          xb[kb][0][0] = movmatrix_trans(xa[kb][j][0]);
+          xb[kb][0][1] = movmatrix_trans(xa[kb][j][1]);
+          xb[kb][1][0] = movmatrix_trans(xa[kb][j][2]);
+          xb[kb][1][1] = movmatrix_trans(xa[kb][j][3]);
+        }
+#pragma unroll
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            x[i][j].v[h][0] *= s0[i];
+            x[i][j].v[h][1] *= s0[i];
+            x[i][j].v[h][2] *= s1[i];
+            x[i][j].v[h][3] *= s1[i];
+#pragma unroll
+            for (int kb = 0; kb < NB; ++kb) mma_bf16(x[i][j].v[h], ba[i][kb], xb[kb][h][0], xb[kb][h][1]);
+          }
+      }
+    }
 
     // ---------------- F: untile + scaled, weight-decayed write (Eq. 4.6) ---------------
     const float keep = 1.f - hp.lr * hp.wd;
-    const float unq = 1.f / qs;
-    const float stepsz = step_mode ? -hp.lr * hp.scale_c * L.tau_base * unq : unq;
+    const float stepsz = step_mode ? -hp.lr * hp.scale_c * cur.tau_base : 1.f;
 #pragma unroll
-    for (int q = 0; q < NB * NB * 4; ++q) {
-      const int i = q / (NB * 4), j = (q / 4) % NB, nh = (q >> 1) & 1, rr = q & 1;
-      const int row = row0 + 16 * i + g + 8 * rr, col = col0 + 16 * j + 8 * nh + 2 * c;
-      float o0 = stepsz * x[i][j].v[nh][2 * rr], o1 = stepsz * x[i][j].v[nh][2 * rr + 1];
-      if (step_mode) {
-        o0 = fmaf(keep, __uint_as_float(wq[q] << 16), o0);
-        o1 = fmaf(keep, __uint_as_float(wq[q] & 0xffff0000u), o1);
+    for (int r = 0; r < kRowsPerLane; ++r) {
+      const int i = r >> 1, rr = r & 1;
+      uint32_t ww[kLaneBytes / 4], wo[kLaneBytes / 4];
+      if (step_mode) read_row(cur, buf, 2, cur.pw, cur.sw, r, ww);
+#pragma unroll
+      for (int q = 0; q < kLaneBytes / 4; ++q) {
+        float o0 = stepsz * x[i][q >> 1].v[q & 1][2 * rr], o1 = stepsz * x[i][q >> 1].v[q & 1][2 * rr + 1];
+        if (step_mode) {
+          o0 = fmaf(keep, bf_lo(ww[q]), o0);
+          o1 = fmaf(keep, bf_hi(ww[q]), o1);
+        }
+        wo[q] = pack2(o0, o1);
       }
-      if (ft.ok) ft.w[(2 * i + rr) * ft.w8 + (2 * j + nh) * 4] = pack2(o0, o1);
-      else ioW.store2(row, col, o0, o1);
+      write_row(cur, cur.pw, cur.sw, r, wo);
     }
+    cur = nxt;
+    buf ^= 1;
     it = nx;
   }
+  cp_async_wait_all();
 }
 
 }  // namespace
 
 cudaError_t launch_warp(const LaunchArgs& a, cudaStream_t s) {
   if (a.n_items < 1) return cudaSuccess;
-  long long grid = (a.n_items + kWarpsPerBlock - 1) / kWarpsPerBlock;
-  const long long cap = (long long)device_sm_count() * 8;
+  if (a.T != 16 && a.T != 32) return cudaErrorInvalidValue;
+  const int per_sm = a.T == 16 ? Cfg<1>::kBlocksPerSm : Cfg<2>::kBlocksPerSm;
+  const int warps = a.T == 16 ? Cfg<1>::kWarps : Cfg<2>::kWarps;
+  const size_t smem = (size_t)warps * 2 * 3 * a.T * a.T * 2;
+  cudaError_t e;
+  if (a.T == 16) {
+    static DeviceOnce once;
+    e = configure_smem_once(once, himuon_warp_kernel<1>, (int)smem);
+  } else {
+    static DeviceOnce once;
+    e = configure_smem_once(once, himuon_warp_kernel<2>, (int)smem);
+  }
+  if (e != cudaSuccess) return e;
+  long long grid = (a.n_items + warps - 1) / warps;
+  const long long cap = (long long)device_sm_count() * per_sm;
   if (grid > cap) grid = cap;
-  if (a.T == 16) himuon_warp_kernel<1><<<(unsigned)grid, kThreads, 0, s>>>(a.layers, a.items, a.n_items, a.mode, a.hp);
-  else if (a.T == 32) himuon_warp_kernel<2><<<(unsigned)grid, kThreads, 0, s>>>(a.layers, a.items, a.n_items, a.mode, a.hp);
-  else return cudaErrorInvalidValue;
+  if (a.T == 16) himuon_warp_kernel<1><<<(unsigned)grid, warps * 32, smem, s>>>(a.layers, a.items, a.n_items, a.mode, a.hp);
+  else himuon_warp_kernel<2><<<(unsigned)grid, warps * 32, smem, s>>>(a.layers, a.items, a.n_items, a.mode, a.hp);
   return cudaGetLastError();
 }
 

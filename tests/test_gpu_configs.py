@@ -156,8 +156,9 @@ def _run_config_w0(spec, T_default, cap_mb, frac, seed, whole_layers, path=hm.HI
         for li in range(n_layers):
             assert torch.equal(Ms[li], Mb[li]), f"layer {li}: M' differs between the bf16 and the fp32 kernel"
             worst_x = max(worst_x, _per_tile_rel_err_gpu(Ws[li], Wb[li], Tl[li]))   # U = -W'/(lr tau): the scale cancels
-        # both sides carry one bf16 output rounding (<= 2^-9 rms each) and the fp32 kernel is within 1e-4 of the oracle
-        assert worst_x <= tol - 2e-3, f"worst tile of all {plan.n_tiles}: bf16 vs fp32 kernel {worst_x:.3e}"
+        # ||U_bf - U_oracle|| <= ||U_bf - U_fp32|| + ||U_fp32 - U_oracle||, and the fp32 kernel's stored result is within
+        # 1e-4 (arithmetic, oracle-pinned) + 2^-9/sqrt(3) = 1.1e-3 (its one bf16 output rounding) of the oracle
+        assert worst_x <= tol - 1.2e-3, f"worst tile of all {plan.n_tiles}: bf16 vs fp32 kernel {worst_x:.3e}"
         pb.destroy()
         del Wb, Mb
     # (3) the oracle-checked tiles, at the north-star tolerance on U itself
@@ -207,10 +208,7 @@ def test_config5_llama3_8b_whole_layers_and_sample_w0():
     assert plan.n_tiles == 425984 and n >= 8448 + 7500
 
 
-@pytest.mark.parametrize("T,frac", [(64, 0.02), (256, 0.02), (32, 0.002),
-                                    pytest.param(16, 0.0005, marks=pytest.mark.xfail(
-                                        strict=False, reason="worst of 27 M tiles at T=16: 3.4e-2 > 3e-2 (tail of the "
-                                        "single-bf16 operand scheme on 16 x 16 tiles); open item"))])
+@pytest.mark.parametrize("T,frac", [(64, 0.02), (256, 0.02), (32, 0.002), (16, 0.0005)])
 def test_config5_llama3_8b_other_tile_sizes_w0(T, frac):
     """The same parameter set at the other tile sizes: a seeded sample vs the oracle (smaller fractions where the
     tile count is in the millions), every tile vs the fp32 kernel where that kernel exists (T <= 128)."""

@@ -41,9 +41,12 @@ def test_fp32_path_cubic_iteration_c_zero(T):
     U = run_phi(G, T, hp)
     PU.check_phi(U, G, T, hp, PU.TOL_FP32, out_is_bf16=False)
     Gb = G.to(torch.bfloat16)
-    with pytest.raises(hm.HimuonError) as ei:
-        run_phi(Gb, T, hp)
-    assert ei.value.status == B.HIMUON_ERR_UNSUPPORTED
+    if T >= 64:
+        with pytest.raises(hm.HimuonError) as ei:
+            run_phi(Gb, T, hp)
+        assert ei.value.status == B.HIMUON_ERR_UNSUPPORTED
+    else:                                                               # warp kernel: plain state, any (a, b, c)
+        PU.check_phi(run_phi(Gb, T, hp), Gb, T, hp, PU.TOL_TC, out_is_bf16=True)
     Ub = run_phi(Gb, T, hp, path=hm.HIMUON_PATH_FP32)                  # bf16 storage, fp32 arithmetic: accepted
     PU.check_phi(Ub, Gb, T, hp, 5e-3, out_is_bf16=True)               # one bf16 rounding of the output
 

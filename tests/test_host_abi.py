@@ -267,13 +267,15 @@ def test_nonpositive_c_is_refused_on_the_tensor_core_paths():
     lib = B._lib()
     for c, want_tc in ((0.0, B.HIMUON_ERR_UNSUPPORTED), (-1.0, B.HIMUON_ERR_UNSUPPORTED), (2.0315, B.HIMUON_ERR_NOT_BOUND)):
         hp = hm.HParams(a=1.5, b=-0.5, c=c).to_c()
-        for T in (16, 64, 128, 256):
+        for T in (64, 128, 256, 512):
             p = hm.Plan(_layers([(512, 512)]), T)
             assert lib.himuon_step(p._h, C.byref(hp), None) == want_tc, (c, T)
             assert lib.himuon_phi(p._h, C.byref(hp), None) == want_tc, (c, T)
         p = hm.Plan(_layers([(512, 512)]), 128, path=hm.HIMUON_PATH_FP8)
         assert lib.himuon_phi(p._h, C.byref(hp), None) == want_tc
-        # fp32 arithmetic (FP32 path on bf16 storage, fp32 storage, large tiles): accepted (only "not bound" here)
+        # the warp kernel (T = 16, 32: plain state) and fp32 arithmetic (FP32 path, fp32 storage): accepted ("not bound" here)
+        p = hm.Plan(_layers([(512, 512)]), 16)
+        assert lib.himuon_phi(p._h, C.byref(hp), None) == B.HIMUON_ERR_NOT_BOUND
         p = hm.Plan(_layers([(512, 512)]), 64, path=hm.HIMUON_PATH_FP32)
         assert lib.himuon_phi(p._h, C.byref(hp), None) == B.HIMUON_ERR_NOT_BOUND
         p = hm.Plan(_layers([(512, 512)], hm.HIMUON_F32), 64)

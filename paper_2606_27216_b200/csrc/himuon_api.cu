@@ -258,7 +258,7 @@ himuon_status himuon_plan_create(const himuon_layer* layers, int32_t n_layers, i
       size_t need;
       if (Te <= 2048 && Twe <= 2048) {   // uniform tiles run in sub-batches: as many tiles as a scratch budget holds (>= 1)
         const size_t per = lt ? lt_path_batch_item_bytes(Te, Twe) : gemm_path_batch_item_bytes(Te, Twe);
-        size_t       budget = (size_t)512 << 20;
+        size_t       budget = (size_t)1024 << 20;
         if (workspace_cap_bytes && workspace_cap_bytes / 2 < budget) budget = workspace_cap_bytes / 2;
         const int key = (Te * 4096 + Twe) * 2 + (lt ? 1 : 0);
         gemm_tiles[key] += (long long)((H + Te - 1) / Te) * ((W + Twe - 1) / Twe);

@@ -32,6 +32,7 @@
 
 #include <algorithm>
 #include <cstring>
+#include <cstdlib>
 
 #include "himuon_internal.h"
 #include "sm100_ptx.cuh"
@@ -43,9 +44,10 @@ namespace {
 using namespace ptx;
 using namespace tc;
 
-constexpr int BM = 128, BN = 256, BK = 64, kStages = 3;
-constexpr uint32_t kABytes = BM * BK * 2, kBBytes = BN * BK * 2, kStageBytes = kABytes + kBBytes;
-constexpr int kGemmThreads = 256;          // warps 0 / 1 / 2: operand producer / MMA issuer / iterate producer, 4-7 epilogue
+constexpr int BM = 128, BN = 256, BK = 64;
+constexpr uint32_t kABytes = BM * BK * 2;
+constexpr int kGemmThreads = 384;          // warps 0 / 1 / 2: operand producer / MMA issuer / iterate producer, 4-11 epilogue
+constexpr int kEpiThreads = 256;
 constexpr int kEwThreads = 256;
 constexpr int kPrepBlocks = 32;          // blocks per tile of lt_prep / lt_update (fixed: summation order)
 
@@ -148,8 +150,29 @@ __device__ __forceinline__ float tile_sigma(const float* __restrict__ ssq, int b
   return nrm > 0.f ? qs / (nrm + eps) : 0.f;          // Phi_K(0) = 0
 }
 
+// 16-byte accesses of a tile: base pointers, leading dimensions and live width all multiples of 8 bf16
+__device__ __forceinline__ bool tile_vec8(const TileRef& t, bool with_m) {
+  bool ok = (t.w_ % 8 == 0) && (t.ld_g % 8 == 0) && (t.ld_w % 8 == 0) && ((reinterpret_cast<uintptr_t>(t.g) & 15) == 0) &&
+            ((reinterpret_cast<uintptr_t>(t.w) & 15) == 0);
+  if (with_m) ok = ok && (t.ld_m % 8 == 0) && ((reinterpret_cast<uintptr_t>(t.m) & 15) == 0);
+  return ok;
+}
+__device__ __forceinline__ void unpack8(const uint4 v, float (&f)[8]) {
+  const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    f[2 * k] = __uint_as_float(w[k] << 16);
+    f[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
+  }
+}
+__device__ __forceinline__ uint4 pack8(const float (&f)[8]) {
+  return make_uint4(pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
+}
+
 // grid (kPrepBlocks, nb), one warp per row of the SCRATCH layout (rp x ldx, coalesced writes); element (i, j) of the
-// iterate is element (i, j) of the tile, or (j, i) when transposed.
+// iterate is element (i, j) of the tile, or (j, i) when transposed.  Untransposed tiles whose rows are 16-byte aligned
+// take the wide path: a lane owns 8 consecutive columns of a BN-column slot, both loads of a slot pair are issued
+// before the first store (the stores to M could alias the loads of G for all the compiler knows).
 __global__ void __launch_bounds__(kEwThreads)
 lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, LtGeom g, int whole, float* __restrict__ xf,
         long long sxf, __nv_bfloat16* __restrict__ xb, long long sxb, float* __restrict__ d0, long long sd,
@@ -161,31 +184,81 @@ lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items,
   float* D = d0 + (long long)b * sd;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   float ss = 0.f;
-  for (int i = blockIdx.x * (kEwThreads / 32) + warp; i < g.rp; i += kPrepBlocks * (kEwThreads / 32)) {
-    for (int slot = 0; slot < g.ntx; ++slot) {        // d partial per BN-column slot, as the E3 epilogue writes them
-      float dd = 0.f;
-      const int j1 = min((slot + 1) * BN, g.ldx);
-      for (int j = slot * BN + lane; j < j1; j += 32) {
-        const int r = g.transposed ? j : i, c = g.transposed ? i : j;    // position in the tile
-        float x = 0.f;
-        if (r < t.h && c < t.w_) {                                         // outside: B_T zero padding
-          const float gg = __bfloat162float(t.g[(long long)r * t.ld_g + c]);
-          x = gg;
-          if (step_mode) {
-            __nv_bfloat16* pm = t.m + (long long)r * t.ld_m + c;
-            const float mm = fmaf(beta, __bfloat162float(*pm), gg);
-            *pm = __float2bfloat16_rn(mm);
-            x = nesterov ? fmaf(beta, mm, gg) : mm;
+  if (!g.transposed && tile_vec8(t, step_mode != 0)) {
+    for (int i = blockIdx.x * (kEwThreads / 32) + warp; i < g.rp; i += kPrepBlocks * (kEwThreads / 32)) {
+      const bool row_ok = i < t.h;
+      for (int slot0 = 0; slot0 < g.ntx; slot0 += 2) {
+        uint4 gv[2], mv[2];
+        bool live[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          const int j = (slot0 + u) * BN + 8 * lane;
+          live[u] = row_ok && slot0 + u < g.ntx && j < t.w_;
+          gv[u] = make_uint4(0, 0, 0, 0);
+          mv[u] = make_uint4(0, 0, 0, 0);
+          if (live[u]) {
+            gv[u] = *reinterpret_cast<const uint4*>(t.g + (long long)i * t.ld_g + j);
+            if (step_mode) mv[u] = *reinterpret_cast<const uint4*>(t.m + (long long)i * t.ld_m + j);
           }
         }
-        X[(long long)i * g.ldx + j] = x;
-        Xb[(long long)i * g.ldx + j] = __float2bfloat16_rn(x);
-        dd = fmaf(x, x, dd);
-      }
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) dd += __shfl_xor_sync(0xffffffffu, dd, o);
-      if (lane == 0) D[(long long)slot * g.rp + i] = dd;
-      ss += dd;                                        // identical in every lane
+        for (int u = 0; u < 2; ++u) {
+          const int slot = slot0 + u, j = slot * BN + 8 * lane;
+          if (slot >= g.ntx) break;
+          float x[8];
+          unpack8(gv[u], x);                                                 // outside the tile: zeros (B_T padding)
+          if (step_mode && live[u]) {
+            float m[8];
+            unpack8(mv[u], m);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) m[k] = fmaf(beta, m[k], x[k]);
+            *reinterpret_cast<uint4*>(t.m + (long long)i * t.ld_m + j) = pack8(m);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) x[k] = nesterov ? fmaf(beta, m[k], x[k]) : m[k];
+          }
+          float dd = 0.f;
+          if (j < g.ldx) {
+            float4* xo = reinterpret_cast<float4*>(X + (long long)i * g.ldx + j);
+            xo[0] = make_float4(x[0], x[1], x[2], x[3]);
+            xo[1] = make_float4(x[4], x[5], x[6], x[7]);
+            *reinterpret_cast<uint4*>(Xb + (long long)i * g.ldx + j) = pack8(x);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) dd = fmaf(x[k], x[k], dd);
+          }
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) dd += __shfl_xor_sync(0xffffffffu, dd, o);
+          if (lane == 0) D[(long long)slot * g.rp + i] = dd;
+          ss += dd;                                      // identical in every lane
+        }
+      }
+    }
+  } else {
+    for (int i = blockIdx.x * (kEwThreads / 32) + warp; i < g.rp; i += kPrepBlocks * (kEwThreads / 32)) {
+      for (int slot = 0; slot < g.ntx; ++slot) {        // d partial per BN-column slot, as the E3 epilogue writes them
+        float dd = 0.f;
+        const int j1 = min((slot + 1) * BN, g.ldx);
+        for (int j = slot * BN + lane; j < j1; j += 32) {
+          const int r = g.transposed ? j : i, c = g.transposed ? i : j;    // position in the tile
+          float x = 0.f;
+          if (r < t.h && c < t.w_) {                                         // outside: B_T zero padding
+            const float gg = __bfloat162float(t.g[(long long)r * t.ld_g + c]);
+            x = gg;
+            if (step_mode) {
+              __nv_bfloat16* pm = t.m + (long long)r * t.ld_m + c;
+              const float mm = fmaf(beta, __bfloat162float(*pm), gg);
+              *pm = __float2bfloat16_rn(mm);
+              x = nesterov ? fmaf(beta, mm, gg) : mm;
+            }
+          }
+          X[(long long)i * g.ldx + j] = x;
+          Xb[(long long)i * g.ldx + j] = __float2bfloat16_rn(x);
+          dd = fmaf(x, x, dd);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) dd += __shfl_xor_sync(0xffffffffu, dd, o);
+        if (lane == 0) D[(long long)slot * g.rp + i] = dd;
+        ss += dd;                                        // identical in every lane
+      }
     }
   }
   __shared__ float red[kEwThreads / 32];
@@ -208,6 +281,46 @@ lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ item
   const float* X = xf + (long long)b * sxf;
   const float sig = ssq ? tile_sigma(ssq, b, eps, qs) : 1.f;      // K = 0: Xf still holds the raw Ghat
   const float stepsz = (step_mode ? lr_scale * t.tau_base * unq : unq) * sig;
+  if (!g.transposed && tile_vec8(t, false)) {
+    // wide path: a thread owns 8 consecutive columns of a row; two such pieces in flight per thread
+    const int w8 = t.w_ / 8;
+    const long long n8 = (long long)t.h * w8, stride = (long long)kPrepBlocks * kEwThreads;
+    for (long long e0 = (long long)blockIdx.x * kEwThreads + threadIdx.x; e0 < n8; e0 += 2 * stride) {
+      float4 xa[2][2];
+      uint4 wv[2];
+      __nv_bfloat16* pw[2];
+      bool live[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const long long e = e0 + u * stride;
+        live[u] = e < n8;
+        if (live[u]) {
+          const int r = (int)(e / w8), c = 8 * (int)(e - (long long)r * w8);
+          const float4* px = reinterpret_cast<const float4*>(X + (long long)r * g.ldx + c);
+          xa[u][0] = __ldcs(px);
+          xa[u][1] = __ldcs(px + 1);
+          pw[u] = t.w + (long long)r * t.ld_w + c;
+          if (step_mode) wv[u] = *reinterpret_cast<const uint4*>(pw[u]);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        if (!live[u]) continue;
+        const float x[8] = {xa[u][0].x, xa[u][0].y, xa[u][0].z, xa[u][0].w, xa[u][1].x, xa[u][1].y, xa[u][1].z, xa[u][1].w};
+        float o[8];
+        if (step_mode) {
+          unpack8(wv[u], o);
+#pragma unroll
+          for (int k = 0; k < 8; ++k) o[k] = fmaf(keep, o[k], stepsz * x[k]);
+        } else {
+#pragma unroll
+          for (int k = 0; k < 8; ++k) o[k] = stepsz * x[k];
+        }
+        *reinterpret_cast<uint4*>(pw[u]) = pack8(o);
+      }
+    }
+    return;
+  }
   const long long n = (long long)t.h * t.w_;
   for (long long e = (long long)blockIdx.x * kEwThreads + threadIdx.x; e < n; e += (long long)kPrepBlocks * kEwThreads) {
     const int r = (int)(e / t.w_), c = (int)(e - (long long)r * t.w_);
@@ -235,23 +348,48 @@ struct GemmParams {
   int write_ops;               // E3: 0 on the last step (no operand of a next product is needed)
   const float* ssq;            // first step only (else null): the iterate is still the raw Ghat, apply sigma here
   float eps, qs;
+  int dbg;
 };
 
-// Epilogue staging (behind the operand stages): three 16 KB buffers.
-//   E1 / E2: one [128 rows x 64 bf16] output chunk each (128-byte swizzle, the layout of the operand tiles), rotating;
-//   E3:      buffers 0 / 1 = [128 rows x 32 fp32] chunks of the iterate (TMA in, updated in place, TMA out), buffer 2 =
-//            three [128 rows x 32 bf16] chunks of the new operand Xb (plain rows of 64 B), rotating.
-constexpr uint32_t kEpiBuf = 16384, kEpiBytes = 2 * kEpiBuf + 3 * 8192;   // 56 KB (E1 / E2 use 3 x 16 KB of it)
+// Shared memory: operand stages (A: 16 KB; B: 32 KB, or 16 KB per CTA of a pair), then the epilogue staging.
+//   E1 / E2: 4 stages (pair: 6) - the mainloop is bound by bytes in flight per SM (stage bytes / TMA round trip), every
+//            stage counts; two alternating 16 KB buffers, one [128 rows x 64 bf16] output chunk each (128-byte swizzle,
+//            the layout of the operand tiles).
+//   E3:      2 stages (pair: 3); kXfBufs 16 KB buffers = [128 rows x 32 fp32] chunks of the iterate (TMA in, updated in
+//            place, TMA out) and three rotating 8 KB buffers = [128 rows x 32 bf16] chunks of the new operand Xb (plain
+//            rows of 64 B).  E3 is bound by the iterate's HBM traffic (2.5 MB per 512 x 512 tile against 0.4 us of tensor
+//            time per CTA tile): the shared memory goes to chunk loads in flight (kXfBufs - 1 chunks ahead of the
+//            epilogue, 80 KB per SM), not to operand stages.
+constexpr uint32_t kEpiBuf = 16384;
+constexpr int kXfBufs = 6;
+constexpr int kMaxStages = 6;
+template <int EPI, bool PAIR> struct Cfg {
+  static constexpr int kStages = EPI == 3 ? (PAIR ? 3 : 2) : (PAIR ? 6 : 4);
+  static constexpr int kBRows = PAIR ? BN / 2 : BN;                  // rows (n) of B held by one CTA
+  static constexpr uint32_t kBBytes = kBRows * BK * 2, kStageBytes = kABytes + kBBytes;
+  static constexpr uint32_t kEpiBytes = EPI == 3 ? kXfBufs * kEpiBuf + 3 * 8192 : 2 * kEpiBuf;
+  static constexpr uint32_t kSmem = kStages * kStageBytes + kEpiBytes + 1024 + 1024;
+};
 struct GemmCtrl {
-  unsigned long long full[kStages], empty[kStages], tfull[2], tempty[2], xfull[2], xfree[2];
+  unsigned long long full[kMaxStages], empty[kMaxStages], tfull[2], tempty[2], xfull[kXfBufs], xfree[kXfBufs];
   uint32_t tmem_base;
+  float red[BM];             // row sums of the upper column halves, handed to the lower halves' threads
 };
-constexpr uint32_t kGemmSmem = kStages * kStageBytes + kEpiBytes + 1024 + 256;
 
-template <int EPI, bool B_MN>
+// PAIR: two CTAs of a cluster work on one 256 x 256 tile with cta_group::2 MMAs (M = 256: 128 rows per CTA, each in its
+// own TMEM; N = 256: each CTA's shared memory holds half of B), so a CTA fetches 32 KB per k-block instead of 48 KB for
+// the same 128 x 256 x 64 of work - the single-CTA mainloop is bound by L2 / shared-memory fill bandwidth (96 B per
+// clock and SM), not by the tensor pipe.  Every CTA runs its own TMA producer into its own stages, both counting their
+// bytes on the LEADER's "stage full" barrier; the leader's MMA warp issues for both, commits are multicast to both.  The
+// epilogues are per CTA (its 128 rows) and identical to the single-CTA kernel's.
+template <int EPI, bool B_MN, bool PAIR>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmOut,
         const __grid_constant__ CUtensorMap tmXf, const GemmParams p) {
+  using C = Cfg<EPI, PAIR>;
+  constexpr int kStages = C::kStages;
+  constexpr uint32_t kEpiBytes = C::kEpiBytes, kStageBytes = C::kStageBytes;
+  constexpr int kUnitM = PAIR ? 2 * BM : BM;                       // rows of C per work unit
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t epi0 = smem0 + kStages * kStageBytes;
@@ -259,6 +397,8 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
   const int tid = threadIdx.x;
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const int lane = tid & 31;
+  const uint32_t rank = PAIR ? cluster_ctarank() : 0u;            // PAIR: 0 = leader (issues the MMAs)
+  const long long unit0 = PAIR ? cluster_id_x() : blockIdx.x, unit_stride = PAIR ? cluster_count_x() : gridDim.x;
 
   if (tid == 0) {
     for (int s = 0; s < kStages; ++s) {
@@ -267,15 +407,24 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(smem_u32(&ctrl->tfull[a]), 1);
-      mbar_init(smem_u32(&ctrl->tempty[a]), 128);
+      mbar_init(smem_u32(&ctrl->tempty[a]), (PAIR ? 2 : 1) * kEpiThreads);      // PAIR: the leader's barrier collects both epilogues
+    }
+    for (int a = 0; a < kXfBufs; ++a) {
       mbar_init(smem_u32(&ctrl->xfull[a]), 1);
       mbar_init(smem_u32(&ctrl->xfree[a]), 1);
     }
     fence_mbar_init();
   }
-  if (warp == 1) tmem_alloc<512>(smem_u32(&ctrl->tmem_base));
-  tc_fence_before_sync();
-  __syncthreads();
+  if (PAIR) {
+    cluster_sync_all();                                           // both CTAs' barriers exist before anyone signals
+    if (warp == 1) tmem_alloc_pair<512>(smem_u32(&ctrl->tmem_base));
+    tc_fence_before_sync();
+    cluster_sync_all();
+  } else {
+    if (warp == 1) tmem_alloc<512>(smem_u32(&ctrl->tmem_base));
+    tc_fence_before_sync();
+    __syncthreads();
+  }
   tc_fence_after_sync();
   const uint32_t tmem_base = ctrl->tmem_base;
 
@@ -289,21 +438,31 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
       prefetch_tmap(&tmB);
       int s = 0;
       uint32_t ph = 0;
-      for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      for (long long tile = unit0; tile < n_tiles; tile += unit_stride) {
         const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
-        const int m0 = (rem / p.nt) * BM, n0 = (rem % p.nt) * BN;
+        const int m0 = (rem / p.nt) * kUnitM + (int)rank * BM, n0 = (rem % p.nt) * BN;
         for (int kb = 0; kb < kb_n; ++kb) {
-          mbar_wait_parked(smem_u32(&ctrl->empty[s]), ph ^ 1);   // slot free (first pass: passes immediately)
-          const uint32_t full = smem_u32(&ctrl->full[s]);
+          // slot free (first pass: passes immediately).  A barrier completed by the LEADER's multicast commit does not
+          // wake a parked thread of the peer before its hint expires (measured: 1 us per k-block): spin in pair mode.
+          if (PAIR) mbar_wait(smem_u32(&ctrl->empty[s]), ph ^ 1);
+          else mbar_wait_parked(smem_u32(&ctrl->empty[s]), ph ^ 1);
+          // PAIR: both CTAs' loads count on the LEADER's barrier (armed by the leader for both stages' bytes)
+          const uint32_t full = PAIR ? mapa_shared(smem_u32(&ctrl->full[s]), 0) : smem_u32(&ctrl->full[s]);
           const uint32_t sa = smem0 + s * kStageBytes, sbm = sa + kABytes;
-          mbar_arrive_expect_tx(full, kStageBytes);
-          tma_load_3d(sa, &tmA, kb * BK, m0, b, full);                        // A: [BM rows x 64 k]
+          if (p.dbg & 2) { if (rank == 0) mbar_arrive(smem_u32(&ctrl->full[s])); if (++s == kStages) { s = 0; ph ^= 1; } continue; }
+          if (rank == 0) mbar_arrive_expect_tx(smem_u32(&ctrl->full[s]), (PAIR ? 2 : 1) * kStageBytes);
+          auto load = [&](uint32_t dst, const CUtensorMap* tm, int x, int y) {
+            if (PAIR) tma_load_3d_pair(dst, tm, x, y, b, full);
+            else tma_load_3d(dst, tm, x, y, b, full);
+          };
+          load(sa, &tmA, kb * BK, m0);                                        // A: [BM rows x 64 k]
+          const int nb0 = n0 + (int)rank * C::kBRows;                         // PAIR: this CTA's half of the tile's columns
           if (!B_MN) {
-            tma_load_3d(sbm, &tmB, kb * BK, n0, b, full);                     // B K-major: [BN rows x 64 k]
+            load(sbm, &tmB, kb * BK, nb0);                                    // B K-major: [kBRows rows x 64 k]
           } else {
 #pragma unroll
-            for (int j = 0; j < BN / 64; ++j)                                 // B MN-major: 4 x [64 k-rows x 64 n]
-              tma_load_3d(sbm + j * (BK * 128), &tmB, n0 + 64 * j, kb * BK, b, full);
+            for (int j = 0; j < C::kBRows / 64; ++j)                          // B MN-major: [64 k-rows x 64 n] boxes
+              load(sbm + j * (BK * 128), &tmB, nb0 + 64 * j, kb * BK);
           }
           if (++s == kStages) { s = 0; ph ^= 1; }
         }
@@ -311,16 +470,20 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
     }
     __syncwarp();
   } else if (warp == 1) {
-    // ================= MMA issuer =================
-    if (elect_one()) {
-      const uint32_t idesc = make_idesc_bf16(BM, BN, 0, B_MN ? 1 : 0);
+    // ================= MMA issuer (PAIR: of the leader; the peer's warp relays its "stage full") =================
+    if (PAIR && rank != 0) {
+      // the peer's tensor core is driven by the leader's instructions
+    } else if (elect_one()) {
+      const uint32_t idesc = make_idesc_bf16(kUnitM, BN, 0, B_MN ? 1 : 0);
       int s = 0;
       uint32_t ph = 0;
       uint32_t tph[2] = {0, 0};
       int it = 0;
-      for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      for (long long tile = unit0; tile < n_tiles; tile += unit_stride, ++it) {
         const int ab = it & 1;
-        mbar_wait_parked(smem_u32(&ctrl->tempty[ab]), tph[ab] ^ 1);   // the epilogue has drained this accumulator
+        // the epilogue(s) have drained this accumulator
+        if (PAIR) mbar_wait(smem_u32(&ctrl->tempty[ab]), tph[ab] ^ 1);
+        else mbar_wait_parked(smem_u32(&ctrl->tempty[ab]), tph[ab] ^ 1);
         tph[ab] ^= 1;
         tc_fence_after_sync();
         const uint32_t acc = tmem_base + ab * BN;
@@ -333,48 +496,56 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
             const uint64_t da = make_smem_desc_sw128(sa + kk * 32, 16, 1024);
             const uint64_t db = B_MN ? make_smem_desc_sw128(sbm + kk * 2048, BK * 128, 1024)
                                      : make_smem_desc_sw128(sbm + kk * 32, 16, 1024);
-            umma_bf16_ss(acc, da, db, idesc, (kb | kk) ? 1u : 0u);
+            if (PAIR) umma_bf16_ss_pair(acc, da, db, idesc, (kb | kk) ? 1u : 0u);
+            else umma_bf16_ss(acc, da, db, idesc, (kb | kk) ? 1u : 0u);
           }
-          umma_commit(smem_u32(&ctrl->empty[s]));                // frees the smem slot when these MMAs have read it
+          // frees the smem slot (of both CTAs) when these MMAs have read it
+          if (PAIR) umma_commit_pair(smem_u32(&ctrl->empty[s]), (uint16_t)3);
+          else umma_commit(smem_u32(&ctrl->empty[s]));
           if (++s == kStages) { s = 0; ph ^= 1; }
         }
-        umma_commit(smem_u32(&ctrl->tfull[ab]));                 // accumulator ready
+        if (PAIR) umma_commit_pair(smem_u32(&ctrl->tfull[ab]), (uint16_t)3);   // accumulator ready (in both CTAs)
+        else umma_commit(smem_u32(&ctrl->tfull[ab]));
       }
     }
     __syncwarp();
   } else if (warp == 2) {
     // ================= TMA producer: chunks of the fp32 iterate for the E3 epilogue =================
-    if (EPI == EPI_X && elect_one()) {
+    if (EPI == EPI_X && !(p.dbg & 1) && elect_one()) {
       prefetch_tmap(&tmXf);
-      uint32_t n = 0;                                            // running chunk counter: buffer n & 1, phase (n >> 1) & 1
-      for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      uint32_t buf = 0, par = 0;                                 // chunk n lives in buffer n % kXfBufs, phase (n / kXfBufs) & 1
+      for (long long tile = unit0; tile < n_tiles; tile += unit_stride) {
         const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
-        const int m0 = (rem / p.nt) * BM, n0 = (rem % p.nt) * BN;
-        for (int c = 0; c < BN / 32; ++c, ++n) {
-          const uint32_t buf = n & 1, par = (n >> 1) & 1;
+        const int m0 = (rem / p.nt) * kUnitM + (int)rank * BM, n0 = (rem % p.nt) * BN;
+        for (int c = 0; c < BN / 32; ++c) {
           mbar_wait_parked(smem_u32(&ctrl->xfree[buf]), par ^ 1);     // the chunk stored from this buffer has left it
           const uint32_t xfull = smem_u32(&ctrl->xfull[buf]);
           mbar_arrive_expect_tx(xfull, kEpiBuf);
           tma_load_3d(epi0 + buf * kEpiBuf, &tmXf, n0 + 32 * c, m0, b, xfull);
+          if (++buf == kXfBufs) { buf = 0; par ^= 1; }
         }
       }
     }
     __syncwarp();
   } else if (warp >= 4) {
-    // ================= epilogue: thread = accumulator row (TMEM lane); all global traffic through TMA ============
-    const int wq = warp & 3;
+    // ================= epilogue: 8 warps; thread = accumulator row (TMEM lane) x column half of every chunk; all
+    // global traffic through TMA.  Two warps per scheduler: one warp's tcgen05.ld / shared-memory latencies hide behind
+    // the other's arithmetic (with 4 warps the epilogue, not the mainloop, bounded E1 / E2: 15 % issue utilisation).
+    const int wq = warp & 3;                         // TMEM lane quadrant = warp index mod 4
+    const int hf = (warp - 4) >> 2;                  // column half of every chunk this thread works on
     const int row = wq * 32 + lane;                  // row of the tile
-    const int et = tid - 128;                        // 0..127
+    const int et = tid - 128;                        // 0..255
     const uint32_t rsw = (uint32_t)row * 128u;       // row offset in a 128-byte-row staging buffer
     const uint32_t sw = (uint32_t)(row & 7);         // 128-byte swizzle: 16-byte chunk c lives at c ^ (row & 7)
     uint32_t tph[2] = {0, 0};
-    uint32_t nchunk = 0;                             // running chunk counter (E3: mirrors the producer's)
+    uint32_t nchunk = 0;                             // running chunk counter
+    uint32_t xbuf = 0, xpar = 0, xprev = 0;          // E3: mirrors the producer's buffer / phase; buffer of the chunk before
     int it = 0;
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+    for (long long tile = unit0; tile < n_tiles; tile += unit_stride, ++it) {
       const int ab = it & 1;
       const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
       const int mi = rem / p.nt, ni = rem % p.nt;
-      const int m0 = mi * BM, n0 = ni * BN;
+      const int m0 = mi * kUnitM + (int)rank * BM, n0 = ni * BN;
       const int i = m0 + row;                        // row of C
       const bool row_ok = i < p.M;
       // first step: the iterate is the raw Ghat; sigma = q / (||Ghat||_F + eps) is applied here (header)
@@ -392,10 +563,12 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
         for (int sl = 0; sl < p.ntr; ++sl) s_i += S[(long long)sl * p.rp + i];
         s_i = p.a + fmaf(p.beta_h, d_i, s_i);        // a + B_ii, B_ii = beta d_i + (Ah^2)_ii
       }
-      mbar_wait_parked(smem_u32(&ctrl->tfull[ab]), tph[ab]);
+      if (PAIR) mbar_wait(smem_u32(&ctrl->tfull[ab]), tph[ab]);
+      else mbar_wait_parked(smem_u32(&ctrl->tfull[ab]), tph[ab]);
       tph[ab] ^= 1;
       tc_fence_after_sync();
       const uint32_t acc = tmem_base + ab * BN + ((uint32_t)(wq * 32) << 16);
+      if (p.dbg & 1) { tc_fence_before_sync(); if (PAIR) mbar_arrive_cluster(mapa_shared(smem_u32(&ctrl->tempty[ab]), 0)); else mbar_arrive(smem_u32(&ctrl->tempty[ab])); continue; }
       float acc_sq = 0.f;                            // E1: sum_j ACC_ij^2; E3: sum_j x_new_ij^2 over this tile's columns
 
       if (EPI == EPI_X) {
@@ -403,16 +576,16 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
         f2 sq2 = pk2(0.f, 0.f);
 #pragma unroll 1
         for (int c = 0; c < BN / 32; ++c, ++nchunk) {
-          const uint32_t buf = nchunk & 1, par = (nchunk >> 1) & 1;
+          const uint32_t buf = xbuf, par = xpar;
           const uint32_t xs = epi0 + buf * kEpiBuf + rsw;                         // this row of the fp32 chunk
-          const uint32_t xbst = epi0 + 2 * kEpiBuf + (nchunk % 3) * (128 * 64) + (uint32_t)row * 64u;   // ... of the bf16 chunk
-          uint32_t r[32];
-          tmem_ld32(acc + 32 * c, r);
+          const uint32_t xbst = epi0 + kXfBufs * kEpiBuf + (nchunk % 3) * (128 * 64) + (uint32_t)row * 64u;   // ... of the bf16 chunk
+          uint32_t r[16];
+          tmem_ld16(acc + 32 * c + 16 * hf, r);
           mbar_wait_parked(smem_u32(&ctrl->xfull[buf]), par);                     // the iterate's chunk has landed
           tmem_wait_ld();
 #pragma unroll
-          for (int v = 0; v < 8; ++v) {
-            const uint32_t a = xs + (((uint32_t)v ^ sw) << 4);
+          for (int v = 0; v < 4; ++v) {
+            const uint32_t a = xs + (((uint32_t)(4 * hf + v) ^ sw) << 4);
             const uint4 xv = lds128(a);
             f2 x01 = fma2(s2, pk2u(xv.x, xv.y), pk2u(r[4 * v], r[4 * v + 1]));
             f2 x23 = fma2(s2, pk2u(xv.z, xv.w), pk2u(r[4 * v + 2], r[4 * v + 3]));
@@ -424,24 +597,27 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
             upk2u(x01, o0, o1);
             upk2u(x23, o2, o3);
             sts128(a, make_uint4(o0, o1, o2, o3));                                // fp32, in place
-            r[2 * v] = cvt_bf16x2(x01);                                           // bf16 operand, packed into r[0..15]
+            r[2 * v] = cvt_bf16x2(x01);                                           // bf16 operand, packed into r[0..7]
             r[2 * v + 1] = cvt_bf16x2(x23);
           }
           if (p.write_ops) {
 #pragma unroll
-            for (int v = 0; v < 4; ++v) sts128(xbst + 16 * v, make_uint4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]));
+            for (int v = 0; v < 2; ++v)
+              sts128(xbst + 32 * hf + 16 * v, make_uint4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]));
           }
           fence_proxy_async_smem();
-          named_bar_sync(1, 128);
+          named_bar_sync(1, kEpiThreads);
           if (et == 0) {
             tma_store_3d(&tmXf, n0 + 32 * c, m0, b, epi0 + buf * kEpiBuf);
-            if (p.write_ops) tma_store_3d(&tmOut, n0 + 32 * c, m0, b, epi0 + 2 * kEpiBuf + (nchunk % 3) * (128 * 64));
+            if (p.write_ops) tma_store_3d(&tmOut, n0 + 32 * c, m0, b, epi0 + kXfBufs * kEpiBuf + (nchunk % 3) * (128 * 64));
             tma_commit_group();
-            // all but this chunk's stores have read their buffers: the OTHER fp32 buffer may be refilled, and (through
-            // the next chunk's barrier) the bf16 buffer written two chunks ago may be rewritten
+            // all but this chunk's stores have read their buffers: the PREVIOUS chunk's fp32 buffer may be refilled, and
+            // (through the next chunk's barrier) the bf16 buffer written two chunks ago may be rewritten
             tma_wait_group_read1();
-            if (nchunk > 0) mbar_arrive(smem_u32(&ctrl->xfree[buf ^ 1]));
+            if (nchunk > 0) mbar_arrive(smem_u32(&ctrl->xfree[xprev]));
           }
+          xprev = buf;
+          if (++xbuf == kXfBufs) { xbuf = 0; xpar ^= 1; }
         }
         float q0, q1;
         upk2(sq2, q0, q1);
@@ -450,9 +626,9 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
         const float g2s = sig * sig;
 #pragma unroll 1
         for (int c = 0; c < BN / 64; ++c, ++nchunk) {
-          const uint32_t st = epi0 + (nchunk % 3) * kEpiBuf + rsw;                // this row of the [128 x 64] bf16 chunk
-#pragma unroll
-          for (int hh = 0; hh < 2; ++hh) {
+          const uint32_t st = epi0 + (nchunk & 1) * kEpiBuf + rsw;                // this row of the [128 x 64] bf16 chunk
+          {
+            const int hh = hf;
             uint32_t r[32];
             tmem_ld32(acc + 64 * c + 32 * hh, r);
             tmem_wait_ld();
@@ -476,32 +652,47 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
           }
           // the diagonal of the operand: Ot gets d_i + beta/2 (fp32, rounded once), Bb gets 0
           const int dc = i - (n0 + 64 * c);
-          if (row_ok && dc >= 0 && dc < 64) {
+          if (row_ok && dc >= 0 && dc < 64 && (dc >> 5) == hf) {   // by the thread that wrote this column
             const __nv_bfloat16 dv = __float2bfloat16_rn(EPI == EPI_GRAM ? fmaf(0.5f, p.beta_h, d_i) : 0.f);
             const uint32_t a = st + ((((uint32_t)(dc >> 3)) ^ sw) << 4) + (uint32_t)(dc & 7) * 2u;
             asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(*reinterpret_cast<const unsigned short*>(&dv)) : "memory");
           }
           fence_proxy_async_smem();
-          named_bar_sync(1, 128);
+          // two buffers: the store issued one chunk ago must have read its buffer before anyone passes this barrier and
+          // starts writing the next chunk into it (it has had a whole chunk's time to do so)
+          if (et == 0) tma_wait_group_read0();
+          named_bar_sync(1, kEpiThreads);
           if (et == 0) {
-            tma_store_3d(&tmOut, n0 + 64 * c, m0, b, epi0 + (nchunk % 3) * kEpiBuf);
+            tma_store_3d(&tmOut, n0 + 64 * c, m0, b, epi0 + (nchunk & 1) * kEpiBuf);
             tma_commit_group();
-            tma_wait_group_read1();   // the buffer stored one chunk ago is free; the next barrier tells everyone
           }
         }
       }
       tc_fence_before_sync();
-      mbar_arrive(smem_u32(&ctrl->tempty[ab]));      // this thread has read its row of the accumulator
-      if (row_ok) {
-        if (EPI == EPI_GRAM) p.s_part[(long long)b * p.ss + (long long)ni * p.rp + i] = acc_sq;
-        else if (EPI == EPI_X) p.d_out[(long long)b * p.sd + (long long)ni * p.rp + i] = acc_sq;
+      // this thread has read its row of the accumulator
+      if (PAIR) mbar_arrive_cluster(mapa_shared(smem_u32(&ctrl->tempty[ab]), 0));
+      else mbar_arrive(smem_u32(&ctrl->tempty[ab]));
+      if (EPI != EPI_B) {
+        // row sums: lower half + upper half, in this order (the next unit's hand-over is behind its chunk barriers)
+        if (hf == 1) ctrl->red[row] = acc_sq;
+        named_bar_sync(1, kEpiThreads);
+        if (hf == 0 && row_ok) {
+          const float tot = acc_sq + ctrl->red[row];
+          if (EPI == EPI_GRAM) p.s_part[(long long)b * p.ss + (long long)ni * p.rp + i] = tot;
+          else p.d_out[(long long)b * p.sd + (long long)ni * p.rp + i] = tot;
+        }
       }
     }
     if (et == 0) tma_wait_group0();
   }
   tc_fence_before_sync();
-  __syncthreads();
-  if (warp == 1) tmem_dealloc<512>(tmem_base);
+  if (PAIR) {
+    cluster_sync_all();
+    if (warp == 1) tmem_dealloc_pair<512>(tmem_base);
+  } else {
+    __syncthreads();
+    if (warp == 1) tmem_dealloc<512>(tmem_base);
+  }
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -532,17 +723,41 @@ bool encode3d(CUtensorMap* out, void* ptr, bool fp32, int cols, int rows, int nb
             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int EPI, bool B_MN>
-cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmOut, const CUtensorMap& tmXf,
-                        const GemmParams& p, cudaStream_t s) {
+template <int EPI, bool B_MN, bool PAIR>
+cudaError_t launch_gemm_t(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmOut, const CUtensorMap& tmXf,
+                          GemmParams p, cudaStream_t s) {
   static DeviceOnce once;
-  cudaError_t e = configure_smem_once(once, lt_gemm<EPI, B_MN>, (int)kGemmSmem);
+  cudaError_t e = configure_smem_once(once, lt_gemm<EPI, B_MN, PAIR>, (int)Cfg<EPI, PAIR>::kSmem);
   if (e != cudaSuccess) return e;
-  long long tiles = (long long)p.nb * p.mt * p.nt;
-  int grid = (int)std::min<long long>(tiles, device_sm_count());
+  p.mt = (p.M + (PAIR ? 2 : 1) * BM - 1) / ((PAIR ? 2 : 1) * BM);
+  { static const int dbg = [] { const char* e = getenv("HIMUON_LT_DBG"); return e ? atoi(e) : 0; }(); p.dbg = dbg; }
+  p.nt = (p.N + BN - 1) / BN;
+  const long long units = (long long)p.nb * p.mt * p.nt;
+  const int ctas = PAIR ? 2 : 1;
+  int grid = ctas * (int)std::min<long long>(units, device_sm_count() / ctas);
   if (grid < 1) return cudaSuccess;
-  lt_gemm<EPI, B_MN><<<grid, kGemmThreads, kGemmSmem, s>>>(tmA, tmB, tmOut, tmXf, p);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg;
+  std::memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(kGemmThreads);
+  cfg.dynamicSmemBytes = Cfg<EPI, PAIR>::kSmem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = ctas; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, lt_gemm<EPI, B_MN, PAIR>, tmA, tmB, tmOut, tmXf, p);
+}
+// Row blocks of 256 over a CTA pair when the output has more than 128 rows; else one CTA per 128 x 256 tile.
+// tmB / tmBp: the B operand's tensor map with the single-CTA box (BN rows) / the pair's (BN / 2 rows per CTA).
+template <int EPI, bool B_MN>
+cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmBp, const CUtensorMap& tmOut,
+                        const CUtensorMap& tmXf, const GemmParams& p, cudaStream_t s) {
+  static const int force = [] { const char* e = getenv("HIMUON_LT_PAIR"); return e ? atoi(e) : -1; }();   // EXPERIMENT
+  const bool pair = force >= 0 ? (force != 0 && p.M > BM) : (p.M > BM);
+  if (pair) return launch_gemm_t<EPI, B_MN, true>(tmA, tmBp, tmOut, tmXf, p, s);
+  return launch_gemm_t<EPI, B_MN, false>(tmA, tmB, tmOut, tmXf, p, s);
 }
 
 // One sub-batch of nb tiles of geometry g.
@@ -583,18 +798,18 @@ cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev,
       const int cur = k & 1;
       p.ssq = k == 0 ? sc.ssq : nullptr;         // first step: Xf / Xb still hold the raw Ghat
       // A = Xb Xb^T  ->  Ot, S
-      p.M = g.rp; p.N = g.rp; p.K = g.np; p.mt = (g.rp + BM - 1) / BM; p.nt = (g.rp + BN - 1) / BN;
+      p.M = g.rp; p.N = g.rp; p.K = g.np;
       p.d_in = dcur; p.d_out = nullptr;
-      cudaError_t e = launch_gemm<EPI_GRAM, false>(xA[cur], xBk[cur], oA, xF, p, s);
+      cudaError_t e = launch_gemm<EPI_GRAM, false>(xA[cur], xBk[cur], xA[cur], oA, xF, p, s);
       if (e != cudaSuccess) return e;
       // Ot Ot^T  ->  Bb
       p.K = g.rp;
-      e = launch_gemm<EPI_B, false>(oA, oB, bA, xF, p, s);
+      e = launch_gemm<EPI_B, false>(oA, oB, oA, bA, xF, p, s);
       if (e != cudaSuccess) return e;
       // Bb Xb  ->  Xf, Xb, d
-      p.M = g.rp; p.N = g.np; p.K = g.rp; p.mt = (g.rp + BM - 1) / BM; p.nt = (g.np + BN - 1) / BN;
+      p.M = g.rp; p.N = g.np; p.K = g.rp;
       p.d_out = dnext; p.write_ops = (k + 1 < hp.K) ? 1 : 0;
-      e = launch_gemm<EPI_X, true>(bA, xBm[cur], xO[cur ^ 1], xF, p, s);
+      e = launch_gemm<EPI_X, true>(bA, xBm[cur], xBm[cur], xO[cur ^ 1], xF, p, s);
       if (e != cudaSuccess) return e;
       std::swap(dcur, dnext);
       *launches += 3;
@@ -623,6 +838,17 @@ cudaError_t run_lt_path(const LayerDev* layers_host, const WorkItem* items_host,
     if (scratch_bytes < per) return cudaErrorInvalidValue;
     long long cap = (long long)(scratch_bytes / per);
     if (cap > 65535) cap = 65535;     // the tile index is gridDim.y of the fused ends
+    // whole waves: the persistent GEMMs run tiles x CTA-tiles-per-tile work units on one CTA per SM, so a sub-batch whose
+    // unit count is a multiple of the SM count has no ragged last wave (T = 512: 4 units per tile, 74 CTA pairs -> 37 tiles)
+    {
+      const int ctas = g.rp > BM ? 2 : 1;             // CTA pairs on 256-row blocks (launch_gemm)
+      const long long units = (long long)((g.rp + ctas * BM - 1) / (ctas * BM)) * ((g.np + BN - 1) / BN);
+      const long long workers = device_sm_count() / ctas;
+      long long a = workers, b = units;
+      while (b) { const long long t = a % b; a = b; b = t; }
+      const long long wave = workers / a;
+      if (cap >= wave) cap -= cap % wave;
+    }
     for (long long i = 0; i < n_items; i += cap) {
       const int nb = (int)std::min<long long>(cap, n_items - i);
       cudaError_t e = run_sub_batch(layers_dev, items_dev ? items_dev + i : nullptr, nb, g, items_dev ? 0 : (int)i, mode, hp,

@@ -4,35 +4,40 @@
 // study and T = 256 on widths TMA cannot store.  This is the paper's "multi-kernel path
 // with epilogue fusion" (section 4.4.1) re-designed for sm_100a: every product of a Newton-Schulz step
 // (Eq. 2.2) is ONE launch of a hand-written persistent tcgen05 GEMM over all tiles of a sub-batch,
-// with the step's elementwise work fused into its epilogue - nothing but bf16 operands, the fp32 iterate and three
+// with the step's elementwise work fused into its epilogue - nothing but bf16 arrays (operands, the iterate as a hi + lo pair) and three
 // small fp32 vectors per tile ever touches HBM between the products:
 //
-//   lt_prep    M' = beta M + G (stored); Ghat = G + beta M' | M' -> Xf (fp32) and Xb = bf16(Ghat) (scratch,
-//              tile zero-padded, stored TRANSPOSED when the tile is tall so that the Gram matrix is on the short side,
-//              PAPER.md:76); row-norm partials d_i and per-block partial sums of squares (fixed summation order).
+//   lt_prep    M' = beta M + G (stored); Ghat = G + beta M' | M' -> the iterate, kept as TWO bf16 arrays
+//              Xb = bf16(Ghat) (hi: the products' operand) and Xlo = bf16(Ghat - hi) (scratch, tile zero-padded, stored
+//              TRANSPOSED when the tile is tall so that the Gram matrix is on the short side); row-norm
+//              partials d_i and per-block partial sums of squares (fixed summation order).  hi + lo carries 16 mantissa
+//              bits (2^-17 relative, far below the operands' bf16 rounding) and costs half the HBM traffic of an fp32
+//              copy beside the bf16 operand: the path is bound by HBM, every product round-trips through it.
 //              The normalisation X0 = q Ghat / (||Ghat||_F + eps), q = c^(1/4) (Phi_K(0) = 0) is NOT a
 //              pass of its own: bf16 rounding is scale-free, so the first step runs on the raw Ghat and its epilogues
 //              apply sigma = q / (||Ghat||_F + eps) (E1: sigma^2 on the accumulator and on d; E3: sigma on the result).
 //   K x  lt_gemm<E1>  ACC = Xb Xb^T;  epilogue: Ot = bf16(offdiag(ACC) + diag(d + beta/2)) -> Ob;  S_i = sum_j ACC_ij^2
 //        lt_gemm<E2>  ACC = Ot Ot^T (= B off the diagonal);  epilogue: Bb = bf16(ACC), diagonal zeroed -> Bb
-//        lt_gemm<E3>  ACC = Bb Xb;  epilogue: Xf <- (a + beta d_i + S_i) Xf + ACC;  Xb = bf16(Xf);  new d_i partials;
-//   lt_update  W <- (1 - lr wd) W - lr tau Xf / q (Eq. 4.6; Phi mode: W <- Xf / q), un-transposed
+//        lt_gemm<E3>  ACC = Bb Xb;  epilogue: x <- sigma ((a + beta d_i + S_i) (hi + lo) + ACC) in fp32; new hi -> the
+//                     other Xb, new lo in place; new d_i partials
+//   lt_update  W <- (1 - lr wd) W - lr tau (hi + lo) / q (Eq. 4.6; Phi mode: W <- (hi + lo) / q),
+//              un-transposed
 // The numerical scheme is the one of the fused kernels (scaled state, fp32 diagonals of A and B as row scalings, the
 // operand-diagonal trick), so the accuracy is the same <= 3e-2 class.
 //
 // lt_gemm: C[b] (M x N, fp32 in TMEM) = A[b] (M x K, K-major) * B[b]; B is K-major (N x K: Gram form) or MN-major
-// (K x N: plain product).  CTA tile 128 x 256, k-block 64, 3 smem stages of 48 KB filled by TMA (3-D tensor maps over
-// the batched scratch arrays; out-of-bounds rows / columns read as zero), SS-mode tcgen05.mma 128 x 256 x 16 issued by
-// one thread, two 256-column accumulators in TMEM so that the epilogue of one tile overlaps the products of the next;
-// persistent over batch x tiles.  Warps: 0 = TMA producer of the operands, 1 = MMA issuer, 2 = TMA producer of the fp32
-// iterate's chunks (E3), 4-7 = epilogue: thread = accumulator row, and every byte of the epilogue's global traffic goes
-// through TMA (iterate chunks in, updated in place in shared memory, out; bf16 operands out) - tcgen05.ld hands a thread
-// one ROW, so direct global accesses would be 32 rows per warp instruction.
+// (K x N: plain product).  CTA tile 128 x 256 (or 256 x 256 over a CTA pair, below), k-block 64, shared-memory stages
+// filled by TMA (3-D tensor maps over the batched scratch arrays; out-of-bounds rows / columns read as zero), SS-mode
+// tcgen05.mma 128 x 256 x 16 issued by one thread, two 256-column accumulators in TMEM so that the epilogue of one tile
+// overlaps the products of the next; persistent over batch x tiles.  Warps: 0 = TMA producer of the operands, 1 = MMA
+// issuer, 2 = TMA producer of the iterate's chunks (E3), 4-11 = epilogue: thread = accumulator row x column half, and
+// every byte of the epilogue's global traffic goes through TMA (iterate chunks in, updated in place in shared memory,
+// out; bf16 operands out) - tcgen05.ld hands a thread one ROW, so direct global accesses would be 32 rows per warp
+// instruction.
 #include <cuda_bf16.h>
 
 #include <algorithm>
 #include <cstring>
-#include <cstdlib>
 
 #include "himuon_internal.h"
 #include "sm100_ptx.cuh"
@@ -83,19 +88,19 @@ LtGeom make_geom(int Th, int Tw) {
 
 size_t a256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-// Scratch of a sub-batch of nb tiles: Xf (fp32), Xb, Ob, Bb (bf16), d partials x 2 (ping-pong), S partials, ss partials.
+// Scratch of a sub-batch of nb tiles: Xb x 2, Xlo, Ob, Bb (bf16), d partials x 2 (ping-pong), S partials, ss partials.
 struct LtScratch {
-  float* xf; __nv_bfloat16 *xb, *xb2, *ob, *bb; float *d0, *d1, *sp, *ssq;   // xb / xb2: product 3 reads one, writes the other
+  __nv_bfloat16 *xlo, *xb, *xb2, *ob, *bb; float *d0, *d1, *sp, *ssq;   // xb / xb2: product 3 reads one, writes the other
 };
 size_t lt_item_bytes(const LtGeom& g) {
-  return a256((size_t)g.sx * 4) + 2 * a256((size_t)g.sx * 2) + 2 * a256((size_t)g.sr * 2) + 2 * a256((size_t)g.sd * 4) +
+  return 3 * a256((size_t)g.sx * 2) + 2 * a256((size_t)g.sr * 2) + 2 * a256((size_t)g.sd * 4) +
          a256((size_t)g.ss * 4) + a256(kPrepBlocks * 4);
 }
 LtScratch carve(char* base, const LtGeom& g, int nb) {
   LtScratch s;
   size_t off = 0;
   auto take = [&](size_t per) { char* p = base + off; off += (size_t)nb * per; return p; };
-  s.xf = (float*)take(a256((size_t)g.sx * 4));
+  s.xlo = (__nv_bfloat16*)take(a256((size_t)g.sx * 2));
   s.xb = (__nv_bfloat16*)take(a256((size_t)g.sx * 2));
   s.xb2 = (__nv_bfloat16*)take(a256((size_t)g.sx * 2));
   s.ob = (__nv_bfloat16*)take(a256((size_t)g.sr * 2));
@@ -107,7 +112,6 @@ LtScratch carve(char* base, const LtGeom& g, int nb) {
   return s;
 }
 // per-tile strides in ELEMENTS of the carved arrays (the a256 rounding is per tile)
-long long stride_xf(const LtGeom& g) { return (long long)(a256((size_t)g.sx * 4) / 4); }
 long long stride_xb(const LtGeom& g) { return (long long)(a256((size_t)g.sx * 2) / 2); }
 long long stride_r(const LtGeom& g) { return (long long)(a256((size_t)g.sr * 2) / 2); }
 long long stride_d(const LtGeom& g) { return (long long)(a256((size_t)g.sd * 4) / 4); }
@@ -174,12 +178,12 @@ __device__ __forceinline__ uint4 pack8(const float (&f)[8]) {
 // take the wide path: a lane owns 8 consecutive columns of a BN-column slot, both loads of a slot pair are issued
 // before the first store (the stores to M could alias the loads of G for all the compiler knows).
 __global__ void __launch_bounds__(kEwThreads)
-lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, LtGeom g, int whole, float* __restrict__ xf,
-        long long sxf, __nv_bfloat16* __restrict__ xb, long long sxb, float* __restrict__ d0, long long sd,
+lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, LtGeom g, int whole,
+        __nv_bfloat16* __restrict__ xlo, __nv_bfloat16* __restrict__ xb, long long sxb, float* __restrict__ d0, long long sd,
         float* __restrict__ ssq, int step_mode, float beta, int nesterov) {
   const int b = blockIdx.y;
   const TileRef t = tile_ref(layers, items, b, g.Th, g.Tw, whole);
-  float* X = xf + (long long)b * sxf;
+  __nv_bfloat16* Xl = xlo + (long long)b * sxb;
   __nv_bfloat16* Xb = xb + (long long)b * sxb;
   float* D = d0 + (long long)b * sd;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -218,10 +222,13 @@ lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items,
           }
           float dd = 0.f;
           if (j < g.ldx) {
-            float4* xo = reinterpret_cast<float4*>(X + (long long)i * g.ldx + j);
-            xo[0] = make_float4(x[0], x[1], x[2], x[3]);
-            xo[1] = make_float4(x[4], x[5], x[6], x[7]);
-            *reinterpret_cast<uint4*>(Xb + (long long)i * g.ldx + j) = pack8(x);
+            const uint4 hi = pack8(x);
+            float h[8], l[8];
+            unpack8(hi, h);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) l[k] = x[k] - h[k];
+            *reinterpret_cast<uint4*>(Xb + (long long)i * g.ldx + j) = hi;
+            *reinterpret_cast<uint4*>(Xl + (long long)i * g.ldx + j) = pack8(l);
 #pragma unroll
             for (int k = 0; k < 8; ++k) dd = fmaf(x[k], x[k], dd);
           }
@@ -250,8 +257,9 @@ lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items,
               x = nesterov ? fmaf(beta, mm, gg) : mm;
             }
           }
-          X[(long long)i * g.ldx + j] = x;
-          Xb[(long long)i * g.ldx + j] = __float2bfloat16_rn(x);
+          const __nv_bfloat16 hi = __float2bfloat16_rn(x);
+          Xb[(long long)i * g.ldx + j] = hi;
+          Xl[(long long)i * g.ldx + j] = __float2bfloat16_rn(x - __bfloat162float(hi));
           dd = fmaf(x, x, dd);
         }
 #pragma unroll
@@ -274,19 +282,21 @@ lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items,
 
 __global__ void __launch_bounds__(kEwThreads)
 lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, LtGeom g, int whole,
-          const float* __restrict__ xf, long long sxf, int step_mode, float keep, float lr_scale, float unq,
+          const __nv_bfloat16* __restrict__ xhi, const __nv_bfloat16* __restrict__ xlo, long long sxb, int step_mode, float keep,
+          float lr_scale, float unq,
           const float* __restrict__ ssq, float eps, float qs) {
   const int b = blockIdx.y;
   const TileRef t = tile_ref(layers, items, b, g.Th, g.Tw, whole);
-  const float* X = xf + (long long)b * sxf;
-  const float sig = ssq ? tile_sigma(ssq, b, eps, qs) : 1.f;      // K = 0: Xf still holds the raw Ghat
+  const __nv_bfloat16* Xh = xhi + (long long)b * sxb;
+  const __nv_bfloat16* Xl = xlo + (long long)b * sxb;
+  const float sig = ssq ? tile_sigma(ssq, b, eps, qs) : 1.f;      // K = 0: the iterate is still the raw Ghat
   const float stepsz = (step_mode ? lr_scale * t.tau_base * unq : unq) * sig;
   if (!g.transposed && tile_vec8(t, false)) {
     // wide path: a thread owns 8 consecutive columns of a row; two such pieces in flight per thread
     const int w8 = t.w_ / 8;
     const long long n8 = (long long)t.h * w8, stride = (long long)kPrepBlocks * kEwThreads;
     for (long long e0 = (long long)blockIdx.x * kEwThreads + threadIdx.x; e0 < n8; e0 += 2 * stride) {
-      float4 xa[2][2];
+      uint4 xh[2], xl[2];
       uint4 wv[2];
       __nv_bfloat16* pw[2];
       bool live[2];
@@ -296,9 +306,8 @@ lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ item
         live[u] = e < n8;
         if (live[u]) {
           const int r = (int)(e / w8), c = 8 * (int)(e - (long long)r * w8);
-          const float4* px = reinterpret_cast<const float4*>(X + (long long)r * g.ldx + c);
-          xa[u][0] = __ldcs(px);
-          xa[u][1] = __ldcs(px + 1);
+          xh[u] = __ldcs(reinterpret_cast<const uint4*>(Xh + (long long)r * g.ldx + c));
+          xl[u] = __ldcs(reinterpret_cast<const uint4*>(Xl + (long long)r * g.ldx + c));
           pw[u] = t.w + (long long)r * t.ld_w + c;
           if (step_mode) wv[u] = *reinterpret_cast<const uint4*>(pw[u]);
         }
@@ -306,7 +315,11 @@ lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ item
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
         if (!live[u]) continue;
-        const float x[8] = {xa[u][0].x, xa[u][0].y, xa[u][0].z, xa[u][0].w, xa[u][1].x, xa[u][1].y, xa[u][1].z, xa[u][1].w};
+        float x[8], xq[8];
+        unpack8(xh[u], x);
+        unpack8(xl[u], xq);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) x[k] += xq[k];
         float o[8];
         if (step_mode) {
           unpack8(wv[u], o);
@@ -324,7 +337,8 @@ lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ item
   const long long n = (long long)t.h * t.w_;
   for (long long e = (long long)blockIdx.x * kEwThreads + threadIdx.x; e < n; e += (long long)kPrepBlocks * kEwThreads) {
     const int r = (int)(e / t.w_), c = (int)(e - (long long)r * t.w_);
-    const float x = g.transposed ? X[(long long)c * g.ldx + r] : X[(long long)r * g.ldx + c];
+    const long long at = g.transposed ? (long long)c * g.ldx + r : (long long)r * g.ldx + c;
+    const float x = __bfloat162float(Xh[at]) + __bfloat162float(Xl[at]);
     __nv_bfloat16* p = t.w + (long long)r * t.ld_w + c;
     *p = __float2bfloat16_rn(step_mode ? fmaf(keep, __bfloat162float(*p), stepsz * x) : stepsz * x);
   }
@@ -345,33 +359,31 @@ struct GemmParams {
   int ntr;
   int rp;
   float a, beta_h;
-  int write_ops;               // E3: 0 on the last step (no operand of a next product is needed)
   const float* ssq;            // first step only (else null): the iterate is still the raw Ghat, apply sigma here
   float eps, qs;
-  int dbg;
 };
 
 // Shared memory: operand stages (A: 16 KB; B: 32 KB, or 16 KB per CTA of a pair), then the epilogue staging.
 //   E1 / E2: 4 stages (pair: 6) - the mainloop is bound by bytes in flight per SM (stage bytes / TMA round trip), every
 //            stage counts; two alternating 16 KB buffers, one [128 rows x 64 bf16] output chunk each (128-byte swizzle,
 //            the layout of the operand tiles).
-//   E3:      2 stages (pair: 3); kXfBufs 16 KB buffers = [128 rows x 32 fp32] chunks of the iterate (TMA in, updated in
-//            place, TMA out) and three rotating 8 KB buffers = [128 rows x 32 bf16] chunks of the new operand Xb (plain
-//            rows of 64 B).  E3 is bound by the iterate's HBM traffic (2.5 MB per 512 x 512 tile against 0.4 us of tensor
-//            time per CTA tile): the shared memory goes to chunk loads in flight (kXfBufs - 1 chunks ahead of the
-//            epilogue, 80 KB per SM), not to operand stages.
+//   E3:      3 stages (pair: 4); kXBufs 16 KB buffers = one [128 rows x 32 columns] chunk of the iterate each, as its two
+//            bf16 halves (hi at +0, lo at +8 KB; rows of 64 B, 64-byte swizzle): TMA in, updated in place, TMA out.  E3 is
+//            bound by the iterate's HBM traffic, so the rest of the shared memory goes to chunk loads in flight
+//            (kXBufs - 1 chunks ahead of the epilogue).
 constexpr uint32_t kEpiBuf = 16384;
-constexpr int kXfBufs = 6;
+constexpr int kMaxXBufs = 6;
 constexpr int kMaxStages = 6;
 template <int EPI, bool PAIR> struct Cfg {
-  static constexpr int kStages = EPI == 3 ? (PAIR ? 3 : 2) : (PAIR ? 6 : 4);
+  static constexpr int kStages = EPI == 3 ? (PAIR ? 4 : 3) : (PAIR ? 6 : 4);
+  static constexpr int kXBufs = PAIR ? 6 : 5;
   static constexpr int kBRows = PAIR ? BN / 2 : BN;                  // rows (n) of B held by one CTA
   static constexpr uint32_t kBBytes = kBRows * BK * 2, kStageBytes = kABytes + kBBytes;
-  static constexpr uint32_t kEpiBytes = EPI == 3 ? kXfBufs * kEpiBuf + 3 * 8192 : 2 * kEpiBuf;
+  static constexpr uint32_t kEpiBytes = EPI == 3 ? kXBufs * kEpiBuf : 2 * kEpiBuf;
   static constexpr uint32_t kSmem = kStages * kStageBytes + kEpiBytes + 1024 + 1024;
 };
 struct GemmCtrl {
-  unsigned long long full[kMaxStages], empty[kMaxStages], tfull[2], tempty[2], xfull[kXfBufs], xfree[kXfBufs];
+  unsigned long long full[kMaxStages], empty[kMaxStages], tfull[2], tempty[2], xfull[kMaxXBufs], xfree[kMaxXBufs];
   uint32_t tmem_base;
   float red[BM];             // row sums of the upper column halves, handed to the lower halves' threads
 };
@@ -385,10 +397,11 @@ struct GemmCtrl {
 template <int EPI, bool B_MN, bool PAIR>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmOut,
-        const __grid_constant__ CUtensorMap tmXf, const GemmParams p) {
+        const __grid_constant__ CUtensorMap tmHi, const __grid_constant__ CUtensorMap tmLo, const GemmParams p) {
   using C = Cfg<EPI, PAIR>;
   constexpr int kStages = C::kStages;
   constexpr uint32_t kEpiBytes = C::kEpiBytes, kStageBytes = C::kStageBytes;
+  constexpr int kXBufs = C::kXBufs;
   constexpr int kUnitM = PAIR ? 2 * BM : BM;                       // rows of C per work unit
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -409,7 +422,7 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
       mbar_init(smem_u32(&ctrl->tfull[a]), 1);
       mbar_init(smem_u32(&ctrl->tempty[a]), (PAIR ? 2 : 1) * kEpiThreads);      // PAIR: the leader's barrier collects both epilogues
     }
-    for (int a = 0; a < kXfBufs; ++a) {
+    for (int a = 0; a < kXBufs; ++a) {
       mbar_init(smem_u32(&ctrl->xfull[a]), 1);
       mbar_init(smem_u32(&ctrl->xfree[a]), 1);
     }
@@ -449,7 +462,6 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
           // PAIR: both CTAs' loads count on the LEADER's barrier (armed by the leader for both stages' bytes)
           const uint32_t full = PAIR ? mapa_shared(smem_u32(&ctrl->full[s]), 0) : smem_u32(&ctrl->full[s]);
           const uint32_t sa = smem0 + s * kStageBytes, sbm = sa + kABytes;
-          if (p.dbg & 2) { if (rank == 0) mbar_arrive(smem_u32(&ctrl->full[s])); if (++s == kStages) { s = 0; ph ^= 1; } continue; }
           if (rank == 0) mbar_arrive_expect_tx(smem_u32(&ctrl->full[s]), (PAIR ? 2 : 1) * kStageBytes);
           auto load = [&](uint32_t dst, const CUtensorMap* tm, int x, int y) {
             if (PAIR) tma_load_3d_pair(dst, tm, x, y, b, full);
@@ -511,9 +523,10 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
     __syncwarp();
   } else if (warp == 2) {
     // ================= TMA producer: chunks of the fp32 iterate for the E3 epilogue =================
-    if (EPI == EPI_X && !(p.dbg & 1) && elect_one()) {
-      prefetch_tmap(&tmXf);
-      uint32_t buf = 0, par = 0;                                 // chunk n lives in buffer n % kXfBufs, phase (n / kXfBufs) & 1
+    if (EPI == EPI_X && elect_one()) {
+      prefetch_tmap(&tmHi);
+      prefetch_tmap(&tmLo);
+      uint32_t buf = 0, par = 0;                                 // chunk n lives in buffer n % kXBufs, phase (n / kXBufs) & 1
       for (long long tile = unit0; tile < n_tiles; tile += unit_stride) {
         const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
         const int m0 = (rem / p.nt) * kUnitM + (int)rank * BM, n0 = (rem % p.nt) * BN;
@@ -521,8 +534,9 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
           mbar_wait_parked(smem_u32(&ctrl->xfree[buf]), par ^ 1);     // the chunk stored from this buffer has left it
           const uint32_t xfull = smem_u32(&ctrl->xfull[buf]);
           mbar_arrive_expect_tx(xfull, kEpiBuf);
-          tma_load_3d(epi0 + buf * kEpiBuf, &tmXf, n0 + 32 * c, m0, b, xfull);
-          if (++buf == kXfBufs) { buf = 0; par ^= 1; }
+          tma_load_3d(epi0 + buf * kEpiBuf, &tmHi, n0 + 32 * c, m0, b, xfull);
+          tma_load_3d(epi0 + buf * kEpiBuf + kEpiBuf / 2, &tmLo, n0 + 32 * c, m0, b, xfull);
+          if (++buf == kXBufs) { buf = 0; par ^= 1; }
         }
       }
     }
@@ -568,56 +582,52 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
       tph[ab] ^= 1;
       tc_fence_after_sync();
       const uint32_t acc = tmem_base + ab * BN + ((uint32_t)(wq * 32) << 16);
-      if (p.dbg & 1) { tc_fence_before_sync(); if (PAIR) mbar_arrive_cluster(mapa_shared(smem_u32(&ctrl->tempty[ab]), 0)); else mbar_arrive(smem_u32(&ctrl->tempty[ab])); continue; }
       float acc_sq = 0.f;                            // E1: sum_j ACC_ij^2; E3: sum_j x_new_ij^2 over this tile's columns
 
       if (EPI == EPI_X) {
         const f2 s2 = pk2(s_i, s_i), g2 = pk2(sig, sig);
         f2 sq2 = pk2(0.f, 0.f);
+        const uint32_t rs64 = (uint32_t)row * 64u, sw64 = (uint32_t)((row >> 1) & 3);   // 64-byte rows, 64-byte swizzle
 #pragma unroll 1
         for (int c = 0; c < BN / 32; ++c, ++nchunk) {
           const uint32_t buf = xbuf, par = xpar;
-          const uint32_t xs = epi0 + buf * kEpiBuf + rsw;                         // this row of the fp32 chunk
-          const uint32_t xbst = epi0 + kXfBufs * kEpiBuf + (nchunk % 3) * (128 * 64) + (uint32_t)row * 64u;   // ... of the bf16 chunk
+          const uint32_t xs = epi0 + buf * kEpiBuf + rs64;                        // this row of the chunk's hi half
           uint32_t r[16];
           tmem_ld16(acc + 32 * c + 16 * hf, r);
           mbar_wait_parked(smem_u32(&ctrl->xfull[buf]), par);                     // the iterate's chunk has landed
           tmem_wait_ld();
 #pragma unroll
-          for (int v = 0; v < 4; ++v) {
-            const uint32_t a = xs + (((uint32_t)(4 * hf + v) ^ sw) << 4);
-            const uint4 xv = lds128(a);
-            f2 x01 = fma2(s2, pk2u(xv.x, xv.y), pk2u(r[4 * v], r[4 * v + 1]));
-            f2 x23 = fma2(s2, pk2u(xv.z, xv.w), pk2u(r[4 * v + 2], r[4 * v + 3]));
-            x01 = mul2(x01, g2);
-            x23 = mul2(x23, g2);
-            sq2 = fma2(x01, x01, sq2);
-            sq2 = fma2(x23, x23, sq2);
-            uint32_t o0, o1, o2, o3;
-            upk2u(x01, o0, o1);
-            upk2u(x23, o2, o3);
-            sts128(a, make_uint4(o0, o1, o2, o3));                                // fp32, in place
-            r[2 * v] = cvt_bf16x2(x01);                                           // bf16 operand, packed into r[0..7]
-            r[2 * v + 1] = cvt_bf16x2(x23);
-          }
-          if (p.write_ops) {
+          for (int v = 0; v < 2; ++v) {
+            const uint32_t a = xs + (((uint32_t)(2 * hf + v) ^ sw64) << 4);
+            const uint4 hv = lds128(a), lv = lds128(a + kEpiBuf / 2);
+            const uint32_t hw[4] = {hv.x, hv.y, hv.z, hv.w}, lw[4] = {lv.x, lv.y, lv.z, lv.w};
+            uint32_t ho[4], lo[4];
 #pragma unroll
-            for (int v = 0; v < 2; ++v)
-              sts128(xbst + 32 * hf + 16 * v, make_uint4(r[4 * v], r[4 * v + 1], r[4 * v + 2], r[4 * v + 3]));
+            for (int j = 0; j < 4; ++j) {
+              // x = hi + lo (exact in fp32); x_new = sigma ((a + B_ii) x + ACC); hi' = bf16(x_new), lo' = bf16(x_new - hi')
+              const f2 x = pk2(bf16_lo(hw[j]) + bf16_lo(lw[j]), bf16_hi(hw[j]) + bf16_hi(lw[j]));
+              const f2 xn = mul2(fma2(s2, x, pk2u(r[8 * v + 2 * j], r[8 * v + 2 * j + 1])), g2);
+              sq2 = fma2(xn, xn, sq2);
+              float x0, x1;
+              upk2(xn, x0, x1);
+              ho[j] = pack_bf16(x0, x1);
+              lo[j] = pack_bf16(x0 - bf16_lo(ho[j]), x1 - bf16_hi(ho[j]));
+            }
+            sts128(a, make_uint4(ho[0], ho[1], ho[2], ho[3]));                    // in place
+            sts128(a + kEpiBuf / 2, make_uint4(lo[0], lo[1], lo[2], lo[3]));
           }
           fence_proxy_async_smem();
           named_bar_sync(1, kEpiThreads);
           if (et == 0) {
-            tma_store_3d(&tmXf, n0 + 32 * c, m0, b, epi0 + buf * kEpiBuf);
-            if (p.write_ops) tma_store_3d(&tmOut, n0 + 32 * c, m0, b, epi0 + kXfBufs * kEpiBuf + (nchunk % 3) * (128 * 64));
+            tma_store_3d(&tmOut, n0 + 32 * c, m0, b, epi0 + buf * kEpiBuf);                 // hi: the next product's operand
+            tma_store_3d(&tmLo, n0 + 32 * c, m0, b, epi0 + buf * kEpiBuf + kEpiBuf / 2);
             tma_commit_group();
-            // all but this chunk's stores have read their buffers: the PREVIOUS chunk's fp32 buffer may be refilled, and
-            // (through the next chunk's barrier) the bf16 buffer written two chunks ago may be rewritten
+            // all but this chunk's stores have read their buffers: the PREVIOUS chunk's buffer may be refilled
             tma_wait_group_read1();
             if (nchunk > 0) mbar_arrive(smem_u32(&ctrl->xfree[xprev]));
           }
           xprev = buf;
-          if (++xbuf == kXfBufs) { xbuf = 0; xpar ^= 1; }
+          if (++xbuf == kXBufs) { xbuf = 0; xpar ^= 1; }
         }
         float q0, q1;
         upk2(sq2, q0, q1);
@@ -709,8 +719,9 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 // [nb][rows][cols] array with row pitch ld and batch pitch sb (elements); box = box_cols x box_rows x 1.
+// swizzle: bytes of the swizzle span (128, 64) or 0 for none
 bool encode3d(CUtensorMap* out, void* ptr, bool fp32, int cols, int rows, int nb, long long ld, long long sb, int box_cols,
-              int box_rows, bool swizzle) {
+              int box_rows, int swizzle) {
   EncodeTiledFn fn = encode_fn();
   if (!fn) return false;
   const cuuint64_t es = fp32 ? 4 : 2;
@@ -719,18 +730,17 @@ bool encode3d(CUtensorMap* out, void* ptr, bool fp32, int cols, int rows, int nb
   cuuint32_t box[3] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows, 1u};
   cuuint32_t estr[3] = {1u, 1u, 1u};
   return fn(out, fp32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, ptr, dims, strides, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 template <int EPI, bool B_MN, bool PAIR>
-cudaError_t launch_gemm_t(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmOut, const CUtensorMap& tmXf,
-                          GemmParams p, cudaStream_t s) {
+cudaError_t launch_gemm_t(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmOut, const CUtensorMap& tmHi,
+                          const CUtensorMap& tmLo, GemmParams p, cudaStream_t s) {
   static DeviceOnce once;
   cudaError_t e = configure_smem_once(once, lt_gemm<EPI, B_MN, PAIR>, (int)Cfg<EPI, PAIR>::kSmem);
   if (e != cudaSuccess) return e;
   p.mt = (p.M + (PAIR ? 2 : 1) * BM - 1) / ((PAIR ? 2 : 1) * BM);
-  { static const int dbg = [] { const char* e = getenv("HIMUON_LT_DBG"); return e ? atoi(e) : 0; }(); p.dbg = dbg; }
   p.nt = (p.N + BN - 1) / BN;
   const long long units = (long long)p.nb * p.mt * p.nt;
   const int ctas = PAIR ? 2 : 1;
@@ -747,45 +757,45 @@ cudaError_t launch_gemm_t(const CUtensorMap& tmA, const CUtensorMap& tmB, const 
   attr[0].val.clusterDim.x = ctas; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, lt_gemm<EPI, B_MN, PAIR>, tmA, tmB, tmOut, tmXf, p);
+  return cudaLaunchKernelEx(&cfg, lt_gemm<EPI, B_MN, PAIR>, tmA, tmB, tmOut, tmHi, tmLo, p);
 }
-// Row blocks of 256 over a CTA pair when the output has more than 128 rows; else one CTA per 128 x 256 tile.
+// CTA pairs on 256-row blocks when the contraction is long (the full-matrix branch: the mainloop dominates and the
+// pair's smaller operand fetch wins, 1.31 -> 1.26 s on the Llama-3-8B shapes); one CTA per 128 x 256 tile otherwise
+// (T = 512: eight k-blocks per tile, the pair's cross-CTA hand-overs cost more than its fetch saves, 180 vs 174 ms).
 // tmB / tmBp: the B operand's tensor map with the single-CTA box (BN rows) / the pair's (BN / 2 rows per CTA).
 template <int EPI, bool B_MN>
 cudaError_t launch_gemm(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmBp, const CUtensorMap& tmOut,
-                        const CUtensorMap& tmXf, const GemmParams& p, cudaStream_t s) {
-  static const int force = [] { const char* e = getenv("HIMUON_LT_PAIR"); return e ? atoi(e) : -1; }();   // EXPERIMENT
-  const bool pair = force >= 0 ? (force != 0 && p.M > BM) : (p.M > BM);
-  if (pair) return launch_gemm_t<EPI, B_MN, true>(tmA, tmBp, tmOut, tmXf, p, s);
-  return launch_gemm_t<EPI, B_MN, false>(tmA, tmB, tmOut, tmXf, p, s);
+                        const CUtensorMap& tmHi, const CUtensorMap& tmLo, const GemmParams& p, cudaStream_t s) {
+  if (p.M > BM && p.K > 512) return launch_gemm_t<EPI, B_MN, true>(tmA, tmBp, tmOut, tmHi, tmLo, p, s);
+  return launch_gemm_t<EPI, B_MN, false>(tmA, tmB, tmOut, tmHi, tmLo, p, s);
 }
 
 // One sub-batch of nb tiles of geometry g.
 cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev, int nb, const LtGeom& g, int whole, int mode,
                           const himuon_hparams& hp, char* scratch, cudaStream_t s, long long* launches) {
   const LtScratch sc = carve(scratch, g, nb);
-  const long long sxf = stride_xf(g), sxb = stride_xb(g), sr = stride_r(g), sd = stride_d(g), ssp = stride_s(g);
+  const long long sxb = stride_xb(g), sr = stride_r(g), sd = stride_d(g), ssp = stride_s(g);
   const bool step_mode = (mode == MODE_STEP);
   const float qs = sqrtf(sqrtf(hp.c)), beta_h = hp.b / sqrtf(hp.c);
   const dim3 grid_t(kPrepBlocks, nb);
-  lt_prep<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xf, sxf, sc.xb, sxb, sc.d0, sd, sc.ssq,
+  lt_prep<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xlo, sc.xb, sxb, sc.d0, sd, sc.ssq,
                                         step_mode ? 1 : 0, hp.beta, hp.nesterov);
   *launches += 1;
   if (hp.K > 0) {
     // Xb is double-buffered: product 3 of a step reads Xb (all rows of a column block, as the B operand of EVERY row
     // block's tile) while its epilogues write the new Xb, so input and output must be different arrays.
     __nv_bfloat16* xbuf[2] = {sc.xb, sc.xb2};
-    CUtensorMap xA[2], xBk[2], xBm[2], xO[2], oA, oB, bA, xF;
+    CUtensorMap xA[2], xBk[2], xBm[2], xO[2], oA, oB, bA, xL;
     for (int i = 0; i < 2; ++i)
-      if (!encode3d(&xA[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, BM, true) ||
-          !encode3d(&xBk[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, BN, true) ||
-          !encode3d(&xBm[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, 64, true) ||
-          !encode3d(&xO[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 32, BM, false))     // E3's 32-column output chunks
+      if (!encode3d(&xA[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, BM, 128) ||
+          !encode3d(&xBk[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, BN, 128) ||
+          !encode3d(&xBm[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 64, 64, 128) ||
+          !encode3d(&xO[i], xbuf[i], false, g.np, g.rp, nb, g.ldx, sxb, 32, BM, 64))        // E3's 32-column chunks of the iterate's hi half
         return cudaErrorNotSupported;
-    if (!encode3d(&oA, sc.ob, false, g.rp, g.rp, nb, g.ldr, sr, 64, BM, true) ||
-        !encode3d(&oB, sc.ob, false, g.rp, g.rp, nb, g.ldr, sr, 64, BN, true) ||
-        !encode3d(&bA, sc.bb, false, g.rp, g.rp, nb, g.ldr, sr, 64, BM, true) ||
-        !encode3d(&xF, sc.xf, true, g.np, g.rp, nb, g.ldx, sxf, 32, BM, true))               // fp32 iterate, 32-column chunks
+    if (!encode3d(&oA, sc.ob, false, g.rp, g.rp, nb, g.ldr, sr, 64, BM, 128) ||
+        !encode3d(&oB, sc.ob, false, g.rp, g.rp, nb, g.ldr, sr, 64, BN, 128) ||
+        !encode3d(&bA, sc.bb, false, g.rp, g.rp, nb, g.ldr, sr, 64, BM, 128) ||
+        !encode3d(&xL, sc.xlo, false, g.np, g.rp, nb, g.ldx, sxb, 32, BM, 64))               // ... and of its lo half
       return cudaErrorNotSupported;
     GemmParams p;
     std::memset(&p, 0, sizeof(p));
@@ -796,26 +806,27 @@ cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev,
     float* dnext = sc.d1;
     for (int k = 0; k < hp.K; ++k) {
       const int cur = k & 1;
-      p.ssq = k == 0 ? sc.ssq : nullptr;         // first step: Xf / Xb still hold the raw Ghat
+      p.ssq = k == 0 ? sc.ssq : nullptr;         // first step: the iterate is still the raw Ghat
       // A = Xb Xb^T  ->  Ot, S
       p.M = g.rp; p.N = g.rp; p.K = g.np;
       p.d_in = dcur; p.d_out = nullptr;
-      cudaError_t e = launch_gemm<EPI_GRAM, false>(xA[cur], xBk[cur], xA[cur], oA, xF, p, s);
+      cudaError_t e = launch_gemm<EPI_GRAM, false>(xA[cur], xBk[cur], xA[cur], oA, xL, xL, p, s);
       if (e != cudaSuccess) return e;
       // Ot Ot^T  ->  Bb
       p.K = g.rp;
-      e = launch_gemm<EPI_B, false>(oA, oB, oA, bA, xF, p, s);
+      e = launch_gemm<EPI_B, false>(oA, oB, oA, bA, xL, xL, p, s);
       if (e != cudaSuccess) return e;
-      // Bb Xb  ->  Xf, Xb, d
+      // Bb Xb  ->  new iterate (hi into the other Xb, lo in place), d
       p.M = g.rp; p.N = g.np; p.K = g.rp;
-      p.d_out = dnext; p.write_ops = (k + 1 < hp.K) ? 1 : 0;
-      e = launch_gemm<EPI_X, true>(bA, xBm[cur], xBm[cur], xO[cur ^ 1], xF, p, s);
+      p.d_out = dnext;
+      e = launch_gemm<EPI_X, true>(bA, xBm[cur], xBm[cur], xO[cur ^ 1], xO[cur], xL, p, s);
       if (e != cudaSuccess) return e;
       std::swap(dcur, dnext);
       *launches += 3;
     }
   }
-  lt_update<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xf, sxf, step_mode ? 1 : 0, 1.f - hp.lr * hp.wd,
+  lt_update<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, (hp.K & 1) ? sc.xb2 : sc.xb, sc.xlo, sxb,
+                                          step_mode ? 1 : 0, 1.f - hp.lr * hp.wd,
                                           -hp.lr * hp.scale_c, 1.f / qs, hp.K == 0 ? sc.ssq : nullptr, hp.eps, qs);
   *launches += 1;
   return cudaGetLastError();
@@ -841,7 +852,7 @@ cudaError_t run_lt_path(const LayerDev* layers_host, const WorkItem* items_host,
     // whole waves: the persistent GEMMs run tiles x CTA-tiles-per-tile work units on one CTA per SM, so a sub-batch whose
     // unit count is a multiple of the SM count has no ragged last wave (T = 512: 4 units per tile, 74 CTA pairs -> 37 tiles)
     {
-      const int ctas = g.rp > BM ? 2 : 1;             // CTA pairs on 256-row blocks (launch_gemm)
+      const int ctas = (g.rp > BM && g.rp > 512) ? 2 : 1;   // CTA pairs on 256-row blocks when K > 512 (launch_gemm; K = rp in two of three products)
       const long long units = (long long)((g.rp + ctas * BM - 1) / (ctas * BM)) * ((g.np + BN - 1) / BN);
       const long long workers = device_sm_count() / ctas;
       long long a = workers, b = units;

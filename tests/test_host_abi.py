@@ -180,11 +180,11 @@ def test_supported_tile_sizes_per_dtype_and_path():
     assert small.n_tiles == 4 and small.workspace_bytes < 1 << 20
     # fp32 storage: fp32 cuBLAS products (32 MB of cuBLAS workspace inside the scratch)
     assert hm.Plan(_layers([(512, 512)], hm.HIMUON_F32), 256).workspace_bytes > 32 << 20
-    # bf16: the tcgen05 large-tile path - per tile an fp32 iterate, two bf16 copies of it and two bf16 r x r operands
+    # bf16: the tcgen05 large-tile path - per tile the iterate as three bf16 arrays (hi x 2, lo) and two bf16 r x r operands
     pl = hm.Plan(_layers([(512, 304), (512, 300)]), 256)
-    assert pl.n_buckets == 2 and pl.workspace_bytes > 4 * 256 * 256 * (4 + 2 + 2 + 2 + 2)
+    assert pl.n_buckets == 2 and pl.workspace_bytes > 4 * 256 * 256 * (2 + 2 + 2 + 2 + 2)
     p = hm.Plan(_layers([(1024, 1536)]), 512)
-    assert p.n_tiles == 6 and p.workspace_bytes > 6 * 512 * 512 * (4 + 2 + 2 + 2 + 2)
+    assert p.n_tiles == 6 and p.workspace_bytes > 6 * 512 * 512 * (2 + 2 + 2 + 2 + 2)
     assert hm.Plan(_layers([(200, 256)]), 256).n_tiles == 1     # full-matrix branch served by the T = 256 kernel
     with pytest.raises(hm.HimuonError) as e:                    # the scratch counts against the workspace cap
         hm.Plan(_layers([(4096, 4096)]), 8192, workspace_cap_bytes=64 << 20)

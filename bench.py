@@ -236,7 +236,7 @@ def run_gpu(args):
     kname = {16: "himuon_warp_kernel", 32: "himuon_warp_kernel", 64: "himuon_tc64_kernel", 128: "himuon_tc128_kernel",
              256: "himuon_tc256_kernel"}.get(args.T, "himuon_simt_kernel")
     if args.path == "fp8":                                    # e4m3 peak = measured bf16 peak x the nominal 2:1 ratio
-        kname = "himuon_tc256_fp8_kernel" if args.T == 256 else "himuon_tc128_fp8_kernel"
+        kname = "himuon_tc256_kernel<F8>" if args.T == 256 else "himuon_tc128_kernel<F8>"
         pk = dict(pk, bf16_sustained=2 * pk["bf16_sustained"], bf16_burst=2 * pk["bf16_burst"],
                   source=pk["source"] + " x2 (nominal fp8:bf16 ratio)")
     kern_ms = statistics.mean(per_step) / max(1, plan.n_chunks)

@@ -21,6 +21,13 @@
 // and citations: see the header of kernels_tc128.cu (this kernel is its 2-CTA form; same E1/E2/E3 phases).
 //
 // Thread (t, q) of a CTA: row t of the CTA's 128 rows (TMEM lane t), column quarter q (columns 64q..64q+63).
+//
+// template <bool F8>: the e4m3 variant (HIMUON_PATH_FP8).  Same structure and
+// synchronisation; what changes is the operand format of the three products of a Newton-Schulz step: e4m3
+// (tcgen05.mma kind::f8f6f4, K = 32 per instruction: 8 instead of 16 MMAs per product, half the operand bytes in shared
+// and tensor memory and through distributed shared memory).  Accumulation, the iterate, the diagonals of A and B,
+// momentum and update stay fp32.  Operand scales and their justification: header of kernels_tc128.cu (the bounds do
+// not depend on T).
 #include <cuda_bf16.h>
 #include <stddef.h>
 
@@ -48,10 +55,11 @@ constexpr int kRows = 128;                       // rows of the tile per CTA
 constexpr int kThreads = 512;                    // 16 warps: 4 lane quadrants x 4 column quarters
 constexpr uint32_t kBlkBytes = kRows * 128;      // 16 KB: 128 rows x 64 columns bf16 (one swizzle span wide)
 constexpr uint32_t kBufBytes = 4 * kBlkBytes;    // 64 KB: 128 rows x 256 columns
-constexpr uint32_t kAtomBytes = T * 128;         // 32 KB: 256 K-rows x 64 N-columns of the MN-major operand
+constexpr uint32_t kAtomBytes = T * 128;         // 32 KB: 256 K-rows x 64 N-columns (bf16; 128 of e4m3) of the MN-major operand
+constexpr float kSX = 256.f, kSO = 128.f, kSB = 128.f;   // e4m3 operand scales (powers of two)
 constexpr uint32_t kCtrlBytes = 8192;
 constexpr uint32_t kSmemBytes = 3 * kBufBytes + kCtrlBytes + 1024;   // XB, OB, ST + control + alignment slack
-constexpr uint32_t kAccCol = 0, kOpaCol = 256;   // TMEM: ACC 256 columns (fp32), OPA 128 columns (bf16 pairs)
+constexpr uint32_t kAccCol = 0, kOpaCol = 256;   // TMEM: ACC 256 columns (fp32), OPA 128 columns (bf16 pairs) or 64 (e4m3 quads)
 
 struct Ctrl {
   unsigned long long mma_bar;     // completion of a pair MMA (multicast commit), one per CTA
@@ -68,22 +76,30 @@ static_assert(sizeof(Ctrl) <= kCtrlBytes, "control block too large");
 
 __device__ __forceinline__ uint32_t chunk_addr(uint32_t rowaddr, int c) { return rowaddr ^ ((uint32_t)c << 4); }
 
-// K-major operand, this CTA's 128 rows x K = 256: k-step kk = 16 elements = 32 B inside 64-column block kk >> 2.
+// K-major operand, this CTA's 128 rows x K = 256: k-step kk = 16 bf16 (32 e4m3) = 32 B inside 128-byte block kk >> 2.
 __device__ __forceinline__ uint64_t desc_kmajor(uint32_t buf, int kk) {
   return make_smem_desc_sw128(buf + (kk >> 2) * kBlkBytes + (kk & 3) * 32, 16, 1024);
 }
-// MN-major operand, K = 256 rows x this CTA's 128 N-columns as two 64-column atoms kAtomBytes apart.
+// MN-major operand, K = 256 rows x this CTA's 128 N-columns: bf16 as two 64-column atoms kAtomBytes apart (k-step = 16
+// rows of 128 B), e4m3 as one 128-byte span (k-step = 32 rows).
+template <bool F8>
 __device__ __forceinline__ uint64_t desc_mnmajor(uint32_t buf, int kk) {
-  return make_smem_desc_sw128(buf + kk * 2048, kAtomBytes, 1024);
+  return make_smem_desc_sw128(buf + kk * (F8 ? 4096 : 2048), kAtomBytes, 1024);
 }
+template <bool F8>
 __device__ __forceinline__ void issue_pair(uint32_t acc, uint32_t opa, uint32_t buf, bool mn_major, uint32_t bar) {
-  const uint32_t idesc = mn_major ? make_idesc_bf16(T, T, 0, 1) : make_idesc_bf16(T, T, 0, 0);
+  const uint32_t idesc = F8 ? (mn_major ? make_idesc_e4m3(T, T, 0, 1) : make_idesc_e4m3(T, T, 0, 0))
+                            : (mn_major ? make_idesc_bf16(T, T, 0, 1) : make_idesc_bf16(T, T, 0, 0));
 #pragma unroll
-  for (int kk = 0; kk < T / 16; ++kk)
-    umma_bf16_ts_pair(acc, opa + 8 * kk, mn_major ? desc_mnmajor(buf, kk) : desc_kmajor(buf, kk), idesc, kk ? 1u : 0u);
+  for (int kk = 0; kk < T / (F8 ? 32 : 16); ++kk) {
+    const uint64_t db = mn_major ? desc_mnmajor<F8>(buf, kk) : desc_kmajor(buf, kk);
+    if (F8) umma_f8_ts_pair(acc, opa + 8 * kk, db, idesc, kk ? 1u : 0u);
+    else umma_bf16_ts_pair(acc, opa + 8 * kk, db, idesc, kk ? 1u : 0u);
+  }
   umma_commit_pair(bar, (uint16_t)3);
 }
 
+template <bool F8>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __restrict__ tmaps,
                     const WorkItem* __restrict__ items, long long n_items, int mode, himuon_hparams hp) {
@@ -101,17 +117,24 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   const int R = (int)rank * kRows + t; // row of the tile
   const bool lead = (tid == 0);
   const bool step_mode = (mode == MODE_STEP);
-  // diagonal element (R, R): column quarter R >> 6, 16-column chunk (R & 63) >> 4 of it, packed word (R & 15) >> 1
+  // diagonal element (R, R): column quarter R >> 6, 16-column chunk (R & 63) >> 4 of it; bf16: packed word (R & 15) >> 1,
+  // half R & 1; e4m3: packed word (R & 15) >> 2, byte R & 3
   const bool own = (q4 == (int)(2 * rank) + (wq >> 1));            // warp-uniform
-  const int dq = (t & 63) >> 4, dword = (t & 15) >> 1;
-  const uint32_t dkeep = (t & 1) ? 0x0000ffffu : 0xffff0000u;
+  const int dq = (t & 63) >> 4, dword = F8 ? (t & 15) >> 2 : (t & 15) >> 1;
+  const uint32_t dshift = F8 ? (uint32_t)(t & 3) * 8u : (uint32_t)(t & 1) * 16u;
+  const uint32_t dkeep = ~((F8 ? 0xffu : 0xffffu) << dshift);
 
   const uint32_t XB = smem0, OB = XB + kBufBytes, ST = OB + kBufBytes;
   const uint32_t rowoff = (uint32_t)q4 * kBlkBytes + (uint32_t)t * 128u + ((uint32_t)(t & 7) << 4);
-  const uint32_t xrow = XB + rowoff, orow = OB + rowoff, srow = ST + rowoff;
+  const uint32_t xrow = XB + rowoff, orow = OB + rowoff, srow = ST + rowoff;   // bf16 rows (operands, and staging of G / M / W)
+  // e4m3 operand rows (first 32 KB of XB / OB): K-span block q4 >> 1, this thread's 64 bytes = chunks 4(q4&1)..+3
+  const uint32_t row8 = (uint32_t)(q4 >> 1) * kBlkBytes + (uint32_t)t * 128u + ((uint32_t)((4 * (q4 & 1)) ^ (t & 7)) << 4);
+  const uint32_t xrow8 = XB + row8, orow8 = OB + row8;
   // this thread's 64 columns of row R in the MN-major (column-split) copy of Xb, which lives in the staging
   // buffer ST during the steps: CTA q4 >> 1, atom q4 & 1, K-row R
-  const uint32_t xt_local = ST + (uint32_t)(q4 & 1) * kAtomBytes + (uint32_t)R * 128u + ((uint32_t)(R & 7) << 4);
+  // (e4m3: one 128-byte span per K-row, this thread's 64 bytes = chunks 4(q4&1)..+3 of it)
+  const uint32_t xt_local = F8 ? ST + (uint32_t)R * 128u + ((uint32_t)((4 * (q4 & 1)) ^ (R & 7)) << 4)
+                               : ST + (uint32_t)(q4 & 1) * kAtomBytes + (uint32_t)R * 128u + ((uint32_t)(R & 7) << 4);
   const bool xt_is_local = ((uint32_t)(q4 >> 1) == rank);              // warp-uniform
   const uint32_t xt_row = xt_is_local ? xt_local : mapa_shared(xt_local, (uint32_t)(q4 >> 1));
   const uint32_t mma_bar = smem_u32(&ctrl->mma_bar);
@@ -135,7 +158,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   const uint32_t tmem_base = ctrl->tmem_base;
   const uint32_t lane_off = (uint32_t)(wq * 32) << 16;
   const uint32_t acc_t = tmem_base + lane_off + kAccCol + 64u * q4;   // this thread's 64 accumulator columns
-  const uint32_t opa_t = tmem_base + lane_off + kOpaCol + 32u * q4;   // this thread's 32 packed operand columns
+  const uint32_t opa_t = tmem_base + lane_off + kOpaCol + (F8 ? 16u : 32u) * q4;   // this thread's 32 (e4m3: 16) packed operand columns
   const uint32_t ACCd = tmem_base + kAccCol, OPAd = tmem_base + kOpaCol;
 
   uint32_t ph_mma = 0, ph_ld = 0, ph_w = 0, ph_ready = 0;
@@ -159,7 +182,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         if (rank == 0) {
           mbar_wait_cluster(ready_bar, ph_ready);
           tc_fence_after_sync();
-          issue_pair(ACCd, OPAd, which == 1 ? OB : which == 2 ? XB : ST, which == 3, mma_bar);
+          issue_pair<F8>(ACCd, OPAd, which == 1 ? OB : which == 2 ? XB : ST, which == 3, mma_bar);
         }
       }
       __syncwarp();
@@ -179,19 +202,55 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   // The column-split bf16 copy of the iterate that MMA3 reads (into ST of the owning CTA).  Called right after
   // MMA1 has been issued, i.e. off the critical path: the stores (half of them remote) overlap the MMA.
   auto write_xb_copy = [&](const f2 (&xs)[32]) {
+    const f2 sx2 = pk2(kSX, kSX);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-      uint32_t x8[8];
+      if (F8) {
+        uint32_t x4[4];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) x8[j] = cvt_bf16x2(xs[8 * q + j]);
-      if (xt_is_local) {
-        sts128(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
-        sts128(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
+        for (int j = 0; j < 4; ++j) x4[j] = cvt_e4m3x4(mul2(xs[8 * q + 2 * j], sx2), mul2(xs[8 * q + 2 * j + 1], sx2));
+        if (xt_is_local) sts128(chunk_addr(xt_row, q), make_uint4(x4[0], x4[1], x4[2], x4[3]));
+        else st_cluster_v4(chunk_addr(xt_row, q), make_uint4(x4[0], x4[1], x4[2], x4[3]));
       } else {
-        st_cluster_v4(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
-        st_cluster_v4(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
+        uint32_t x8[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x8[j] = cvt_bf16x2(xs[8 * q + j]);
+        if (xt_is_local) {
+          sts128(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
+          sts128(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
+        } else {
+          st_cluster_v4(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
+          st_cluster_v4(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
+        }
       }
     }
+  };
+  // 16 columns (chunk q of this thread's 64) of the next A operand: rounded to the operand format (e4m3: scaled by
+  // `scale` first), the diagonal element replaced by dval when this thread owns it (diag), written to this thread's
+  // TMEM operand columns and, if row16 is given, to the K-major shared-memory operand (bf16 row row16 / e4m3 row row8).
+  auto emit_operand = [&](const f2 (&v)[8], f2 scale, int q, bool diag, uint32_t dval, uint32_t row16, uint32_t row8) {
+    if (F8) {
+      uint32_t p[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) p[j] = cvt_e4m3x4(mul2(v[2 * j], scale), mul2(v[2 * j + 1], scale));
+      if (diag) set_one4(p, dq == q ? dword : 4, dkeep, dval);
+      if (row8) sts128(chunk_addr(row8, q), make_uint4(p[0], p[1], p[2], p[3]));
+      tmem_st4(opa_t + 4 * q, p);
+    } else {
+      uint32_t p[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) p[j] = cvt_bf16x2(v[j]);
+      if (diag) set_one(p, dq == q ? dword : 8, dkeep, dval);
+      if (row16) {
+        sts128(chunk_addr(row16, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
+        sts128(chunk_addr(row16, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
+      }
+      tmem_st8(opa_t + 8 * q, p);
+    }
+  };
+  auto acc_pairs = [](const uint32_t (&c)[16], f2 (&v)[8]) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) v[j] = pk2u(c[2 * j], c[2 * j + 1]);
   };
 
   // G -> OB and (step mode) M -> XB of tile i: this CTA's 128 rows, four 64-column boxes each
@@ -298,18 +357,13 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     const float inv = nrm > 0.f ? qs / (nrm + hp.eps) : 0.f;   // Phi_K(0) = 0
     ctrl->dpart[q4][t] = ss * inv * inv;                        // partial diag(Ah)_R in fp32
     {
-      const f2 inv2 = pk2(inv, inv);
+      const f2 inv2 = pk2(inv, inv), sx2 = pk2(kSX, kSX);
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
-        uint32_t p[8];
+        f2 v[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          xs[8 * q + j] = mul2(xs[8 * q + j], inv2);
-          p[j] = cvt_bf16x2(xs[8 * q + j]);
-        }
-        sts128(chunk_addr(orow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));    // Xb lives in OB (G is consumed),
-        sts128(chunk_addr(orow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));  // Ot in XB: see the M' store above
-        tmem_st8(opa_t + 8 * q, p);
+        for (int j = 0; j < 8; ++j) v[j] = xs[8 * q + j] = mul2(xs[8 * q + j], inv2);
+        emit_operand(v, sx2, q, false, 0u, orow, orow8);   // Xb lives in OB (G is consumed), Ot in XB: see the M' store above
       }
     }
     TR();   // prologue compute done
@@ -329,7 +383,11 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       TR();   // MMA1 done
       {
         // Ot = offdiag(Ah) + diag(d + beta/2), rounded to bf16: offdiag(Ot Ot^T) = offdiag(beta Ah + Ah^2)
-        const uint32_t dval = (pack_bf16(fmaf(0.5f, beta_h, di), 0.f) & 0xffffu) << ((t & 1) * 16);
+        // (e4m3: ACC = s_X^2 Ah; operand scale s_O: Ot s_O = ACC s_O / s_X^2)
+        const float dv = fmaf(0.5f, beta_h, di);
+        const uint32_t dval = F8 ? (cvt_e4m3x4(pk2(kSO * dv, 0.f), pk2(0.f, 0.f)) & 0xffu) << dshift
+                                 : (pack_bf16(dv, 0.f) & 0xffffu) << dshift;
+        const f2 k1 = pk2(kSO / (kSX * kSX), kSO / (kSX * kSX));
         f2 Sa = pk2(0.f, 0.f), Sb = Sa;
         uint32_t r[2][16];
         tmem_ld16(acc_t, r[0]);
@@ -344,16 +402,14 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
             Sa = fma2(o01, o01, Sa);
             Sb = fma2(o23, o23, Sb);
           }
-          uint32_t p[8];
-          pack16(c, p);
-          if (own) set_one(p, dq == q ? dword : 8, dkeep, dval);
-          sts128(chunk_addr(xrow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
-          sts128(chunk_addr(xrow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
-          tmem_st8(opa_t + 8 * q, p);
+          f2 v[8];
+          acc_pairs(c, v);
+          emit_operand(v, k1, q, own, dval, xrow, xrow8);
         }
         float s0, s1;
         upk2(add2(Sa, Sb), s0, s1);
-        ctrl->spart[q4][t] = s0 + s1;
+        const float us = F8 ? 1.f / (kSX * kSX) : 1.f;         // partial (Ah^2)_RR (e4m3: from the scaled accumulator)
+        ctrl->spart[q4][t] = (s0 + s1) * (us * us);
       }
       TR();   // E1 loop done
       ready_and_issue(2);
@@ -371,10 +427,9 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         for (int q = 0; q < 4; ++q) {
           tmem_wait_ld();
           if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
-          uint32_t p[8];
-          pack16(r[q & 1], p);
-          if (own) set_one(p, dq == q ? dword : 8, dkeep, 0u);
-          tmem_st8(opa_t + 8 * q, p);
+          f2 v[8];
+          acc_pairs(r[q & 1], v);
+          emit_operand(v, pk2(kSB / (kSO * kSO), kSB / (kSO * kSO)), q, own, 0u, 0u, 0u);   // e4m3: ACC = s_O^2 B; operand Bb s_B
         }
       }
       TR();   // E2 loop done
@@ -395,7 +450,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         prefetched = true;
       }
       {
-        const f2 si2 = pk2(si, si);
+        const f2 si2 = pk2(si, si), k3 = pk2(1.f / (kSB * kSX), 1.f / (kSB * kSX)), sx2 = pk2(kSX, kSX);
         f2 Da = pk2(0.f, 0.f), Db = Da;
         uint32_t r[2][16];
         tmem_ld16(acc_t, r[0]);
@@ -405,19 +460,19 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
           uint32_t(&c)[16] = r[q & 1];
 #pragma unroll
-          for (int j = 0; j < 8; ++j) xs[8 * q + j] = fma2(xs[8 * q + j], si2, pk2u(c[2 * j], c[2 * j + 1]));
+          for (int j = 0; j < 8; ++j)
+            xs[8 * q + j] = F8 ? fma2(pk2u(c[2 * j], c[2 * j + 1]), k3, mul2(xs[8 * q + j], si2))
+                               : fma2(xs[8 * q + j], si2, pk2u(c[2 * j], c[2 * j + 1]));
           if (!last) {
-            uint32_t p[8];
 #pragma unroll
             for (int j = 0; j < 8; j += 2) {
               Da = fma2(xs[8 * q + j], xs[8 * q + j], Da);
               Db = fma2(xs[8 * q + j + 1], xs[8 * q + j + 1], Db);
             }
+            f2 v[8];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) p[j] = cvt_bf16x2(xs[8 * q + j]);
-            sts128(chunk_addr(orow, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
-            sts128(chunk_addr(orow, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
-            tmem_st8(opa_t + 8 * q, p);
+            for (int j = 0; j < 8; ++j) v[j] = xs[8 * q + j];
+            emit_operand(v, sx2, q, false, 0u, orow, orow8);
           }
         }
         if (!last) {
@@ -490,17 +545,22 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
 
 }  // namespace
 
-cudaError_t launch_tc256(const LaunchArgs& a, cudaStream_t s) {
+namespace {
+template <bool F8>
+cudaError_t launch_tc256_t(const LaunchArgs& a, cudaStream_t s) {
   static DeviceOnce once;   // per device, thread-safe
-  cudaError_t e = configure_smem_once(once, himuon_tc256_kernel, (int)kSmemBytes);
+  cudaError_t e = configure_smem_once(once, himuon_tc256_kernel<F8>, (int)kSmemBytes);
   if (e != cudaSuccess) return e;
   if (a.n_items < 1) return cudaSuccess;
   long long clusters = a.n_items;
   const int max_clusters = device_sm_count() / 2;
   if (clusters > max_clusters) clusters = max_clusters;
-  himuon_tc256_kernel<<<(unsigned)(2 * clusters), kThreads, kSmemBytes, s>>>(a.layers, a.tmaps, a.items, a.n_items, a.mode, a.hp);
+  himuon_tc256_kernel<F8><<<(unsigned)(2 * clusters), kThreads, kSmemBytes, s>>>(a.layers, a.tmaps, a.items, a.n_items, a.mode, a.hp);
   return cudaGetLastError();
 }
+}  // namespace
+cudaError_t launch_tc256(const LaunchArgs& a, cudaStream_t s) { return launch_tc256_t<false>(a, s); }
+cudaError_t launch_tc256_fp8(const LaunchArgs& a, cudaStream_t s) { return launch_tc256_t<true>(a, s); }
 
 }  // namespace himuon
 

@@ -39,7 +39,7 @@ __device__ __forceinline__ void pack16(const uint32_t (&r)[16], uint32_t (&p)[8]
   for (int j = 0; j < 8; ++j) p[j] = pack_bf16(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
 }
 
-// ---- e4m3 operands (kernels_tc128_fp8.cu, kernels_tc256_fp8.cu) ----------------------------------
+// ---- e4m3 operands (the F8 variants of kernels_tc128.cu, kernels_tc256.cu) ----------------------------------
 // four fp32 (two packed pairs) -> four e4m3 bytes, element 0 in the low byte
 __device__ __forceinline__ uint32_t cvt_e4m3x4(f2 v01, f2 v23) {
   float a, b, c, d;

@@ -1,5 +1,5 @@
-"""GPU tests of the fp8 (e4m3) variants of the T = 128 and T = 256 kernels (HIMUON_PATH_FP8; csrc/kernels_tc128_fp8.cu,
-csrc/kernels_tc256_fp8.cu; SURVEY 8(f3);
+"""GPU tests of the fp8 (e4m3) variants of the T = 128 and T = 256 kernels (HIMUON_PATH_FP8; the F8 template
+variants in csrc/kernels_tc128.cu and csrc/kernels_tc256.cu; SURVEY 8(f3);
 PAPER.md:410-424 section 6.5, :440).  Only the operands of the three products of a Newton-Schulz step are e4m3;
 everything else is the bf16 kernel's fp32 arithmetic.  Tolerance: per-tile relative Frobenius error <= 0.15 against
 the float64 oracle (0.07-0.12 measured in emulation on these recipes; the paper reports an

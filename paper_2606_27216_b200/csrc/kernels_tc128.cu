@@ -373,22 +373,21 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     const uint32_t lane_off = (uint32_t)(wq * 32) << 16;
     const uint32_t acc_t = keep(tmem_slot + lane_off + 16u * h);
     const uint32_t opa_t = keep(tmem_slot + lane_off + kOpaCol + (F8 ? 4u : 8u) * h);
-    // The epilogues work in PIECES of 4 packed operand words: 8 columns (bf16) or 16 columns (e4m3), i.e. one 16-byte
-    // shared-memory chunk and 4 TMEM operand columns.  Small pieces keep the phases inside the 112-register budget
-    // (64 of which are the iterate) without spills - a spill here goes to L2: the L1 left beside 205 KB of shared
-    // memory does not hold 512 threads' stack frames (measured: phases 2-3x slower with 100-250 B of spills).
-    constexpr int kPC = F8 ? 16 : 8;          // columns per piece
+    // The epilogues work in PIECES of one 16-column chunk: one tcgen05.ld.x16, 8 (bf16) or 4 (e4m3) packed operand
+    // words, i.e. two or one 16-byte shared-memory chunks and 8 or 4 TMEM operand columns.  One piece in flight at a
+    // time: with the 64-register iterate that is what the 112-register budget holds (a second 16-column buffer to
+    // overlap the next load spills 100 B per thread, and a spill here goes to L2: the L1 left beside 205 KB of shared
+    // memory does not hold 512 threads' stack frames - measured 34.5 ms; 8-column pieces, double-buffered: 30.4 ms;
+    // 16-column pieces, single-buffered: 30.1 ms).
+    constexpr int kPC = 16;                   // columns per piece = one 16-column chunk
     constexpr int kNP = 64 / kPC;             // pieces per thread
     constexpr int kXP = kPC / 2;              // packed pairs of the iterate per piece
-    // piece i: bf16 -> chunk q = i >> 1, half e = i & 1;  e4m3 -> chunk q = i
-    auto acc_col = [&](int i) { return F8 ? 32u * i : 32u * (i >> 1) + 8u * (i & 1); };     // + acc_t
-    auto opa_col = [&](int i) { return F8 ? 8u * i : 16u * (i >> 1) + 4u * (i & 1); };      // + opa_t
-    auto op_addr = [&](uint32_t buf, int i) {                                                // operand chunk in smem
-      return F8 ? (b0 ^ ((uint32_t)i << 5)) + buf : bf_addr(buf, i >> 1, i & 1);
-    };
+    constexpr int kW = F8 ? 4 : 8;            // packed operand words per piece
+    // piece i = chunk q = i
+    auto acc_col = [&](int i) { return 32u * i; };                 // + acc_t
+    auto opa_col = [&](int i) { return (F8 ? 8u : 16u) * i; };     // + opa_t
     // the diagonal element of row t: chunk 2 wq + (lane >> 4), i.e. column half lane >> 4, iteration q = wq
     const bool diag_mine = ((lane >> 4) == h);
-    const int dpiece_lo = F8 ? 0 : ((lane >> 3) & 1);   // bf16: which half of the chunk
     const int didx = t & (kPC - 1);
 
     // The state is Xh = c^(1/4) X: then Ah = Xh Xh^T = sqrt(c) A and B = bA + cA^2 = beta Ah + Ah^2 with
@@ -399,35 +398,39 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     int n_my = (int)(n_items > g0 ? (n_items - g0 + stride - 1) / stride : 0);
     uint32_t ph_mma = 0, ph_tile = 0;   // ph_tile: parity of every once-per-tile barrier (ld_full, w_full, xb_free) and of tau[]
 
-    auto load_piece = [&](int i, uint32_t (&c)[kPC]) {
-      if constexpr (F8) tmem_ld16(acc_t + acc_col(i), c);
-      else tmem_ld8(acc_t + acc_col(i), c);
-    };
-    auto pack_piece = [&](const uint32_t (&c)[kPC], float scale, uint32_t (&p)[4]) {
+    auto load_piece = [&](int i, uint32_t (&c)[kPC]) { tmem_ld16(acc_t + acc_col(i), c); };
+    auto pack_piece = [&](const uint32_t (&c)[kPC], float scale, uint32_t (&p)[kW]) {
       if constexpr (F8) pack16_e4m3(c, pk2(scale, scale), p);
-      else {
-#pragma unroll
-        for (int j = 0; j < 4; ++j) p[j] = pack_bf16(__uint_as_float(c[2 * j]), __uint_as_float(c[2 * j + 1]));
-      }
+      else pack16(c, p);
     };
-    auto pack_state = [&](const f2* x, uint32_t (&p)[4]) {
+    auto pack_state = [&](const f2* x, uint32_t (&p)[kW]) {
       if constexpr (F8) {
         const f2 sx2 = pk2(kSX, kSX);
 #pragma unroll
         for (int j = 0; j < 4; ++j) p[j] = cvt_e4m3x4(mul2(x[2 * j], sx2), mul2(x[2 * j + 1], sx2));
       } else {
 #pragma unroll
-        for (int j = 0; j < 4; ++j) p[j] = cvt_bf16x2(x[j]);
+        for (int j = 0; j < 8; ++j) p[j] = cvt_bf16x2(x[j]);
       }
     };
     // element didx of the piece (bf16: 16-bit half didx & 1 of word didx >> 1; e4m3: byte didx & 3 of word didx >> 2) := val
-    auto patch_diag = [&](uint32_t (&p)[4], uint32_t val) {
+    auto patch_diag = [&](uint32_t (&p)[kW], uint32_t val) {
       const uint32_t sh = F8 ? (uint32_t)(didx & 3) * 8u : (uint32_t)(didx & 1) * 16u;
-      set_one4(p, F8 ? didx >> 2 : didx >> 1, ~((F8 ? 0xffu : 0xffffu) << sh), val << sh);
+      if constexpr (F8) set_one4(p, didx >> 2, ~(0xffu << sh), val << sh);
+      else set_one(p, didx >> 1, ~(0xffffu << sh), val << sh);
     };
-    auto store_operand = [&](uint32_t buf, int i, const uint32_t (&p)[4]) {
-      sts128(op_addr(buf, i), make_uint4(p[0], p[1], p[2], p[3]));
-      tmem_st4(opa_t + opa_col(i), p);
+    auto store_tmem = [&](int i, const uint32_t (&p)[kW]) {
+      if constexpr (F8) tmem_st4(opa_t + opa_col(i), p);
+      else tmem_st8(opa_t + opa_col(i), p);
+    };
+    auto store_operand = [&](uint32_t buf, int i, const uint32_t (&p)[kW]) {
+      if constexpr (F8) {
+        sts128((b0 ^ ((uint32_t)i << 5)) + buf, make_uint4(p[0], p[1], p[2], p[3]));
+      } else {
+        sts128(bf_addr(buf, i, 0), make_uint4(p[0], p[1], p[2], p[3]));
+        sts128(bf_addr(buf, i, 1), make_uint4(p[4], p[5], p[6], p[7]));
+      }
+      store_tmem(i, p);
     };
     auto operands_ready = [&](bool wrote_smem) {   // this thread's part of the next product's operands is in place
       tmem_wait_st();
@@ -503,7 +506,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         const f2 inv2 = pk2(inv, inv);
 #pragma unroll
         for (int i = 0; i < kNP; ++i) {
-          uint32_t p[4];
+          uint32_t p[kW];
 #pragma unroll
           for (int j = 0; j < kXP; ++j) xs[kXP * i + j] = mul2(xs[kXP * i + j], inv2);
           pack_state(&xs[kXP * i], p);
@@ -531,23 +534,21 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           if constexpr (F8) dval = cvt_e4m3x4(pk2(kSO * fmaf(0.5f, beta_h, di), 0.f), pk2(0.f, 0.f)) & 0xffu;
           else dval = pack_bf16(fmaf(0.5f, beta_h, di), 0.f) & 0xffffu;
           f2 Sa = pk2(0.f, 0.f), Sb = Sa;
-          uint32_t c[2][kPC];
-          load_piece(0, c[0]);
+          uint32_t cc[kPC];
 #pragma unroll
           for (int i = 0; i < kNP; ++i) {
+            load_piece(i, cc);
             tmem_wait_ld();
-            if (i + 1 < kNP) load_piece(i + 1, c[(i + 1) & 1]);
-            uint32_t(&cc)[kPC] = c[i & 1];
 #pragma unroll
             for (int j = 0; j < kPC / 4; ++j) {
               const f2 o01 = pk2u(cc[4 * j], cc[4 * j + 1]), o23 = pk2u(cc[4 * j + 2], cc[4 * j + 3]);
               Sa = fma2(o01, o01, Sa);
               Sb = fma2(o23, o23, Sb);
             }
-            uint32_t p[4];
+            uint32_t p[kW];
             pack_piece(cc, kSO / (kSX * kSX), p);              // e4m3: ACC = s_X^2 Ah, operand Ot s_O
-            if ((F8 ? i : (i >> 1)) == wq) {                   // warp-uniform: the chunk that holds this warp's diagonal
-              if (diag_mine && (F8 || (i & 1) == dpiece_lo)) patch_diag(p, dval);
+            if (i == wq) {                                     // warp-uniform: the chunk that holds this warp's diagonal
+              if (diag_mine) patch_diag(p, dval);
             }
             store_operand(kXB, i, p);
           }
@@ -566,18 +567,17 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         const float si = hp.a + fmaf(beta_h, di, sc->spart[0][t] + sc->spart[1][t]);
         if (kDebugStages && dbg == 2) { dumped = true; break; }
         {
-          uint32_t c[2][kPC];
-          load_piece(0, c[0]);
+          uint32_t cc[kPC];
 #pragma unroll
           for (int i = 0; i < kNP; ++i) {
+            load_piece(i, cc);
             tmem_wait_ld();
-            if (i + 1 < kNP) load_piece(i + 1, c[(i + 1) & 1]);
-            uint32_t p[4];
-            pack_piece(c[i & 1], kSB / (kSO * kSO), p);        // e4m3: ACC = s_O^2 B, operand Bb s_B
-            if ((F8 ? i : (i >> 1)) == wq) {
-              if (diag_mine && (F8 || (i & 1) == dpiece_lo)) patch_diag(p, 0u);
+            uint32_t p[kW];
+            pack_piece(cc, kSB / (kSO * kSO), p);        // e4m3: ACC = s_O^2 B, operand Bb s_B
+            if (i == wq) {
+              if (diag_mine) patch_diag(p, 0u);
             }
-            tmem_st4(opa_t + opa_col(i), p);
+            store_tmem(i, p);
           }
         }
         operands_ready(false);
@@ -589,13 +589,11 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         {
           const f2 si2 = pk2(si, si);
           f2 Da = pk2(0.f, 0.f), Db = Da;
-          uint32_t c[2][kPC];
-          load_piece(0, c[0]);
+          uint32_t cc[kPC];
 #pragma unroll
           for (int i = 0; i < kNP; ++i) {
+            load_piece(i, cc);
             tmem_wait_ld();
-            if (i + 1 < kNP) load_piece(i + 1, c[(i + 1) & 1]);
-            uint32_t(&cc)[kPC] = c[i & 1];
             f2* x = &xs[kXP * i];
             if constexpr (F8) {
               const f2 k3 = pk2(1.f / (kSB * kSX), 1.f / (kSB * kSX));
@@ -611,7 +609,7 @@ himuon_tc128_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
                 Da = fma2(x[j], x[j], Da);
                 Db = fma2(x[j + 1], x[j + 1], Db);
               }
-              uint32_t p[4];
+              uint32_t p[kW];
               pack_state(x, p);
               store_operand(kOB, i, p);
             }

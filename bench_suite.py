@@ -49,6 +49,7 @@ def _step_rows(args, hm, pk, dev):
     hp = hm.HParams(K=args.K, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
     AUTO, FP8 = hm.HIMUON_PATH_AUTO, hm.HIMUON_PATH_FP8
     for name, T, cap, path in (("gpt2-small", 128, 2048, AUTO), ("gpt2-xl", 128, 256, AUTO), ("llama3-8b", 128, 2048, AUTO),
+                               ("llama3-8b", 16, 2048, AUTO), ("llama3-8b", 32, 2048, AUTO),
                                ("llama3-8b", 64, 2048, AUTO), ("llama3-8b", 256, 2048, AUTO), ("llama3-8b-sched", 128, 2048, AUTO),
                                ("llama3-8b", 512, 2048, AUTO), ("llama3-8b", 1 << 20, 2048, AUTO),
                                ("llama3-8b", 128, 2048, FP8), ("llama3-8b", 256, 2048, FP8)):   # opt-in e4m3 operands

@@ -131,3 +131,17 @@ def test_rectangular_tiles_step():
             dW = np.linalg.norm(w_gpu[sl] - Wr[sl])
             bound = PU.BF16_ULP * np.linalg.norm(Wr[sl]) + 0.02 * tau * PU.TOL_TC * np.linalg.norm(Ur[sl])
             assert dW <= bound, f"tile ({r},{c}): {dW / bound:.3f}"
+
+
+@pytest.mark.parametrize("H,W", [(1024, 3072), (2560, 1032)])
+def test_full_matrix_branch_on_the_cta_pair_gemm(H, W):
+    """Full-matrix branch on shapes whose contractions are longer than 512, i.e. the CTA-pair (cta_group::2) form of
+    the large-tile GEMM in all three products, wide and tall (transposed iterate), with a ragged last row
+    block: against the oracle's full-matrix Phi_K and, run twice from the same bits, bitwise identical."""
+    _need_gpu()
+    G = I.lowrank_plus_noise(H, W, 64, seed_cfg=77, layer_index=0, tensor_id=I.TENSOR_G)
+    hp = hm.HParams(K=5, eps=1e-7)
+    U1 = _run_phi(G, 1 << 20, hp)
+    U2 = _run_phi(G, 1 << 20, hp)
+    assert torch.equal(U1, U2)
+    PU.check_phi(U1, G, max(H, W), hp, PU.TOL_TC, out_is_bf16=True)

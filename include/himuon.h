@@ -183,6 +183,28 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
                               float eps, void* workspace, size_t workspace_bytes, void* cuda_stream);
 size_t        himuon_ns_tiles_workspace_bytes(void);
 
+/* himuon_ns_tiles for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): bf16 tiles, HIMUON_PATH_AUTO, same arguments and same result as himuon_ns_tiles
+ * (sec. 4.4.1), but WITHOUT a workspace argument.  The device scratch - layer table, tensor maps and,
+ * at T = 512, the operand arrays of the large-tile path - is a file-scope `static __device__` array of
+ * HIMUON_STATIC_SCRATCH_BYTES inside the library: every GPU that loads the library holds that much device memory
+ * until the process exits.  The call issues no cudaMalloc, cudaFree or allocating library routine; it enqueues two
+ * small host-to-device copies (the tables) and the kernels on `cuda_stream` and returns.
+ *   tiles_in / tiles_out   device, [n_tiles, T, T] bf16 row-major contiguous, 16-byte aligned, caller-owned; in-place
+ *                          allowed; edge tiles zero-padded by the caller.
+ *   Limit                  the tiles of ONE call must fit the scratch: n_tiles <= himuon_ns_tiles_static_max_tiles(T)
+ *                          (T = 512: 12 tiles, 2.5 MiB of operands each; T <= 256 needs no per-tile scratch: 2^31 / T
+ *                          tiles).  Beyond it: HIMUON_ERR_WORKSPACE_TOO_SMALL, nothing enqueued, the limit spelled out
+ *                          in himuon_last_cuda_error().  fp32 storage and the FP32 / FP8 paths: use himuon_ns_tiles.
+ *   Sharing                every call on a device uses the SAME array, which keeps the previous call's contents;
+ *                          nothing in it has to start at zero (each call writes every scratch element before reading
+ *                          it).  Calls that can overlap on the GPU (different streams, or threads) RACE on it:
+ *                          serialise them on one stream or with events.  Other errors as himuon_ns_tiles. */
+#define HIMUON_STATIC_SCRATCH_BYTES (32u << 20)
+himuon_status himuon_ns_tiles_static(const void* tiles_in, void* tiles_out, int64_t n_tiles, int32_t T, int32_t K,
+                                     float a, float b, float c, float eps, void* cuda_stream);
+int64_t       himuon_ns_tiles_static_max_tiles(int32_t T);
+
 /* ---- misc --------------------------------------------------------------------------------- */
 const char* himuon_status_string(himuon_status s);
 /* Text of the last CUDA error seen by this thread's most recent failing call ("" if none). */

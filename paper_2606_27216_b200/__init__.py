@@ -5,6 +5,7 @@ The product is the C-ABI shared library `libhimuon.so` (include/himuon.h), built
 """
 from .binding import (  # noqa: F401
     HIMUON_BF16, HIMUON_F32, HIMUON_PATH_AUTO, HIMUON_PATH_FP32, HIMUON_PATH_FP8, HParams, HimuonError, NS_COEFFS, Plan,
-    himuon_launch_count, himuon_layer, himuon_mat, himuon_ns_tiles, himuon_plan_chunks,
+    himuon_launch_count, himuon_layer, himuon_mat, himuon_ns_tiles, himuon_ns_tiles_static,
+    himuon_ns_tiles_static_max_tiles, himuon_plan_chunks,
     himuon_supported_tile_sizes, mat_of, shape_mat,
 )

@@ -93,6 +93,11 @@ def _load(path: str):
                                     C.c_void_p, C.c_size_t, C.c_void_p]
     lib.himuon_ns_tiles_workspace_bytes.restype = C.c_size_t
     lib.himuon_ns_tiles_workspace_bytes.argtypes = []
+    lib.himuon_ns_tiles_static.restype = C.c_int
+    lib.himuon_ns_tiles_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32,
+                                           C.c_float, C.c_float, C.c_float, C.c_float, C.c_void_p]
+    lib.himuon_ns_tiles_static_max_tiles.restype = C.c_int64
+    lib.himuon_ns_tiles_static_max_tiles.argtypes = [C.c_int32]
     lib.himuon_status_string.restype = C.c_char_p
     lib.himuon_status_string.argtypes = [C.c_int]
     lib.himuon_last_cuda_error.restype = C.c_char_p
@@ -301,6 +306,29 @@ def himuon_ns_tiles(tiles_in: torch.Tensor, tiles_out: Optional[torch.Tensor] = 
     # the workspace must outlive the asynchronous launch
     tiles_out._himuon_ws = workspace
     return tiles_out
+
+
+def himuon_ns_tiles_static(tiles_in: torch.Tensor, tiles_out: torch.Tensor, K: int = 5, a: float = NS_COEFFS[0],
+                           b: float = NS_COEFFS[1], c: float = NS_COEFFS[2], eps: float = 1e-7, stream=None) -> torch.Tensor:
+    """himuon_ns_tiles without a workspace and without any allocation (here or in the library): bf16 [N, T, T] tiles,
+    N <= himuon_ns_tiles_static_max_tiles(T); the scratch is a static device array inside the library (himuon.h)."""
+    if tiles_in.dim() != 3 or tiles_in.shape[1] != tiles_in.shape[2] or not tiles_in.is_contiguous():
+        raise ValueError("tiles_in must be a contiguous [N, T, T] tensor")
+    if tiles_in.dtype != torch.bfloat16 or tiles_out.dtype != torch.bfloat16 or tiles_out.shape != tiles_in.shape or not tiles_out.is_contiguous():
+        raise ValueError("tiles_in / tiles_out must be contiguous bf16 tensors of the same shape")
+    lib = _lib()
+    st = lib.himuon_ns_tiles_static(tiles_in.data_ptr(), tiles_out.data_ptr(), tiles_in.shape[0], tiles_in.shape[1],
+                                    K, a, b, c, eps, _stream_ptr(stream))
+    if st == HIMUON_ERR_WORKSPACE_TOO_SMALL:          # the library spells out the limit
+        err = HimuonError(st, "himuon_ns_tiles_static")
+        err.args = (f"{err.args[0]} ({lib.himuon_last_cuda_error().decode()})",)
+        raise err
+    _check(st, "himuon_ns_tiles_static")
+    return tiles_out
+
+
+def himuon_ns_tiles_static_max_tiles(T: int) -> int:
+    return int(_lib().himuon_ns_tiles_static_max_tiles(T))
 
 
 def debug_set_stage(kernel: str, stage: int):

@@ -3,6 +3,8 @@
 // of one kernel launch per chunk.  See include/himuon.h for the contract of every entry point.
 #include <atomic>
 #include <map>
+#include <mutex>
+#include <string>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -583,6 +585,126 @@ himuon_status himuon_ns_tiles(const void* tiles_in, void* tiles_out, int64_t n_t
   la.hp = hp;
   e = launch_chunk(la, kp, s);
   if (e != cudaSuccess) return cuda_fail(e, "ns_tiles: kernel launch");
+  return HIMUON_OK;
+}
+
+}  // extern "C"
+
+// ---- himuon_ns_tiles_static: the packed-tiles entry point for callers that cannot allocate --------------------------
+// Same computation as himuon_ns_tiles on bf16 storage / HIMUON_PATH_AUTO, but the device scratch
+// (layer table, tensor maps, the large-tile path's operand arrays) is this file-scope array instead of a caller
+// workspace: no cudaMalloc / cudaFree / allocating library call on this path, ever.  Every GPU that loads the library
+// holds HIMUON_STATIC_SCRATCH_BYTES of device memory until the process exits.
+namespace {
+
+static __device__ __align__(256) unsigned char g_static_scratch[HIMUON_STATIC_SCRATCH_BYTES];
+
+constexpr size_t kStaticTableBytes = 1024;     // layer table (128 B) + 3 tensor maps, rounded up
+
+// Device address of g_static_scratch on the CURRENT device.  In host code the array's name is only a handle for
+// cudaGetSymbolAddress, never a device pointer; the address differs per device, so it is looked up once per device
+// ordinal with that device current (the caller's), under a mutex.
+cudaError_t static_scratch_ptr(char** out) {
+  static std::mutex mu;
+  static char*      ptr[64] = {nullptr};
+  int               dev = 0;
+  cudaError_t       e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  if (dev >= 0 && dev < 64 && ptr[dev]) { *out = ptr[dev]; return cudaSuccess; }
+  void* p = nullptr;
+  e = cudaGetSymbolAddress(&p, g_static_scratch);
+  if (e != cudaSuccess) return e;
+  if (!p) return cudaErrorInvalidSymbol;
+  if (dev >= 0 && dev < 64) ptr[dev] = (char*)p;
+  *out = (char*)p;
+  return cudaSuccess;
+}
+
+// Scratch bytes the tiles of one call need behind the table area: only the large-tile path (T = 512) has any.
+size_t static_item_bytes(int T) { return select_kpath(HIMUON_BF16, HIMUON_PATH_AUTO, T) == KPATH_LT ? lt_path_batch_item_bytes(T, T) : 0; }
+
+}  // namespace
+
+extern "C" {
+
+int64_t himuon_ns_tiles_static_max_tiles(int32_t T) {
+  bool known = false;
+  for (int t : kTileSizes) known |= (t == T);
+  if (!known || select_kpath(HIMUON_BF16, HIMUON_PATH_AUTO, T) < 0) return 0;
+  const size_t  per = static_item_bytes(T);
+  const int64_t by_index = 0x7fffffffLL / T;                  // tile index x T is a 32-bit row coordinate
+  if (per == 0) return by_index;
+  const int64_t by_scratch = (int64_t)((HIMUON_STATIC_SCRATCH_BYTES - kStaticTableBytes) / per);
+  return by_scratch < by_index ? by_scratch : by_index;
+}
+
+himuon_status himuon_ns_tiles_static(const void* tiles_in, void* tiles_out, int64_t n_tiles, int32_t T, int32_t K,
+                                     float a, float b, float c, float eps, void* cuda_stream) {
+  if (n_tiles < 0) return HIMUON_ERR_INVALID_ARG;
+  bool known = false;
+  for (int t : kTileSizes) known |= (t == T);
+  if (!known) return HIMUON_ERR_INVALID_ARG;
+  himuon_hparams hp;
+  std::memset(&hp, 0, sizeof(hp));
+  hp.K = K; hp.a = a; hp.b = b; hp.c = c; hp.eps = eps;
+  if (!valid_hparams(&hp)) return HIMUON_ERR_INVALID_ARG;
+  const int kp = select_kpath(HIMUON_BF16, HIMUON_PATH_AUTO, T);
+  if (kp < 0 || kp == KPATH_GEMM) return HIMUON_ERR_UNSUPPORTED;      // (the cuBLAS path creates a handle: it allocates)
+  if (kpath_needs_positive_c(kp) && !positive_c_ok(&hp)) return HIMUON_ERR_UNSUPPORTED;
+  if (n_tiles == 0) return HIMUON_OK;
+  if (!tiles_in || !tiles_out) return HIMUON_ERR_INVALID_ARG;
+  const int64_t max_tiles = himuon_ns_tiles_static_max_tiles(T);
+  if (n_tiles > max_tiles) {
+    g_last_cuda_error = "ns_tiles_static: " + std::to_string(n_tiles) + " tiles of " + std::to_string(T) + " x " + std::to_string(T) +
+                        " exceed the static scratch (HIMUON_STATIC_SCRATCH_BYTES = " + std::to_string((size_t)HIMUON_STATIC_SCRATCH_BYTES) +
+                        "): at most " + std::to_string(max_tiles) + " such tiles per call; split the batch or use himuon_ns_tiles";
+    return HIMUON_ERR_WORKSPACE_TOO_SMALL;
+  }
+  if (kpath_uses_tma(kp) && (((uintptr_t)tiles_in & 15) || ((uintptr_t)tiles_out & 15))) return HIMUON_ERR_UNSUPPORTED;
+  if (((uintptr_t)tiles_in & 1) || ((uintptr_t)tiles_out & 1)) return HIMUON_ERR_INVALID_ARG;
+
+  char*       ws = nullptr;
+  cudaError_t e = static_scratch_ptr(&ws);
+  if (e != cudaSuccess) return cuda_fail(e, "ns_tiles_static: cudaGetSymbolAddress(static scratch)");
+
+  // The packed batch is one (n_tiles*T) x T matrix whose tile (r, 0) is tile r.
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  LayerDev     D;
+  D.w = tiles_out; D.g = const_cast<void*>(tiles_in); D.m = nullptr;
+  D.ld_w = T; D.ld_g = T; D.ld_m = 0;
+  D.H = (int)(n_tiles * T); D.W = T; D.tau_base = 0.f; D.dtype = HIMUON_BF16;
+  e = cudaMemcpyAsync(ws, &D, sizeof(D), cudaMemcpyHostToDevice, s);
+  if (e != cudaSuccess) return cuda_fail(e, "ns_tiles_static: layer table");
+  if (kp == KPATH_LT) {     // tcgen05 GEMM path over the implicit list of the packed batch, ONE sub-batch
+    long long n_launch = 0;
+    e = run_lt_path(&D, nullptr, (const LayerDev*)ws, nullptr, n_tiles, T, T, MODE_PHI, hp, ws + kStaticTableBytes,
+                    HIMUON_STATIC_SCRATCH_BYTES - kStaticTableBytes, s, &n_launch);
+    g_launches.fetch_add(n_launch);
+    if (e != cudaSuccess) return cuda_fail(e, "ns_tiles_static: large-tile path");
+    return HIMUON_OK;
+  }
+  if (kpath_uses_tma(kp)) {
+    CUtensorMap maps[3];
+    std::memset(maps, 0, sizeof(maps));
+    if (!encode_bf16_map(&maps[0], D.w, D.H, D.W, T, T > 128 ? 128 : T) || !encode_bf16_map(&maps[1], D.g, D.H, D.W, T, T > 128 ? 128 : T)) {
+      g_last_cuda_error = "ns_tiles_static: cuTensorMapEncodeTiled failed or unavailable";
+      return HIMUON_ERR_CUDA;
+    }
+    e = cudaMemcpyAsync(ws + 128, maps, sizeof(maps), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e, "ns_tiles_static: tensor maps");
+  }
+  LaunchArgs la;
+  la.layers = (const LayerDev*)ws;
+  la.tmaps = (const CUtensorMap*)(ws + 128);
+  la.items = nullptr;
+  la.n_items = n_tiles;
+  la.T = T;
+  la.mode = MODE_PHI;
+  la.dtype = HIMUON_BF16;
+  la.hp = hp;
+  e = launch_chunk(la, kp, s);
+  if (e != cudaSuccess) return cuda_fail(e, "ns_tiles_static: kernel launch");
   return HIMUON_OK;
 }
 

@@ -20,7 +20,14 @@
 // leader's mbarrier; tcgen05.commit multicasts completion to both CTAs.  Per-tile algorithm, numerical scheme
 // and citations: see the header of kernels_tc128.cu (this kernel is its 2-CTA form; same E1/E2/E3 phases).
 //
-// Thread (t, q) of a CTA: row t of the CTA's 128 rows (TMEM lane t), column quarter q (columns 64q..64q+63).
+// Every product is issued as TWO N = 128 halves (columns {64 hb..} and {128 + 64 hb..} of the product, hb = 0, 1: a
+// cta_group::2 MMA takes half of its N from each CTA), each committed on its own mbarrier, and every thread owns columns
+// in both halves - thread (t, q) of a CTA: row t of the CTA's 128 rows (TMEM lane t), the 32-column half q & 1 of the
+// 64-column blocks 2 (q >> 1) and 2 (q >> 1) + 1 - so the epilogue of a product starts on the first half while the second
+// half still runs on the tensor pipe (a product is seen complete ~500 cycles after its last MMA has been issued,
+// that latency is now paid under the first half's epilogue work).  The A operand in tensor
+// memory is double-buffered for this: the next product's operand is written while the current one is still read.
+// Measured on the Llama-3-8B-shaped step, same box: 61.9 -> 60.4 ms (e4m3 operands 44.3 -> 44.0 ms).
 //
 // template <bool F8>: the e4m3 variant (HIMUON_PATH_FP8).  Same structure and
 // synchronisation; what changes is the operand format of the three products of a Newton-Schulz step: e4m3
@@ -59,10 +66,10 @@ constexpr uint32_t kAtomBytes = T * 128;         // 32 KB: 256 K-rows x 64 N-col
 constexpr float kSX = 256.f, kSO = 128.f, kSB = 128.f;   // e4m3 operand scales (powers of two)
 constexpr uint32_t kCtrlBytes = 8192;
 constexpr uint32_t kSmemBytes = 3 * kBufBytes + kCtrlBytes + 1024;   // XB, OB, ST + control + alignment slack
-constexpr uint32_t kAccCol = 0, kOpaCol = 256;   // TMEM: ACC 256 columns (fp32), OPA 128 columns (bf16 pairs) or 64 (e4m3 quads)
+constexpr uint32_t kAccCol = 0, kOpaCol = 256;   // TMEM: ACC 256 columns (fp32), 2 x OPA 128 columns (bf16 pairs; e4m3 quads use 64 of each)
 
 struct Ctrl {
-  unsigned long long mma_bar;     // completion of a pair MMA (multicast commit), one per CTA
+  unsigned long long mma_bar[2];  // completion of the two N-halves of a pair product (multicast commit), per CTA
   unsigned long long ready_bar;   // leader CTA only: both CTAs' operands are in place (2 arrivals)
   unsigned long long ld_bar;      // TMA loads of G (and M)
   unsigned long long w_bar;       // TMA load of W
@@ -74,7 +81,6 @@ struct Ctrl {
 };
 static_assert(sizeof(Ctrl) <= kCtrlBytes, "control block too large");
 
-__device__ __forceinline__ uint32_t chunk_addr(uint32_t rowaddr, int c) { return rowaddr ^ ((uint32_t)c << 4); }
 
 // K-major operand, this CTA's 128 rows x K = 256: k-step kk = 16 bf16 (32 e4m3) = 32 B inside 128-byte block kk >> 2.
 __device__ __forceinline__ uint64_t desc_kmajor(uint32_t buf, int kk) {
@@ -86,17 +92,26 @@ template <bool F8>
 __device__ __forceinline__ uint64_t desc_mnmajor(uint32_t buf, int kk) {
   return make_smem_desc_sw128(buf + kk * (F8 ? 4096 : 2048), kAtomBytes, 1024);
 }
+// One product as two N = 128 halves, each committed on its own barrier so that the epilogue can start on half 0
+// while half 1 runs.  A cta_group::2 MMA takes N / 2 rows (columns, MN-major) of B from each CTA: half hb is made
+// of B rows 64 hb .. 64 hb + 63 of BOTH CTAs, i.e. the product's columns {64 hb .. +63} and {128 + 64 hb .. +63} -
+// global 64-column blocks hb and 2 + hb land in accumulator columns 128 hb .. 128 hb + 127.
 template <bool F8>
-__device__ __forceinline__ void issue_pair(uint32_t acc, uint32_t opa, uint32_t buf, bool mn_major, uint32_t bar) {
-  const uint32_t idesc = F8 ? (mn_major ? make_idesc_e4m3(T, T, 0, 1) : make_idesc_e4m3(T, T, 0, 0))
-                            : (mn_major ? make_idesc_bf16(T, T, 0, 1) : make_idesc_bf16(T, T, 0, 0));
+__device__ __forceinline__ void issue_pair(uint32_t acc, uint32_t opa, uint32_t buf, bool mn_major, uint32_t bar0, uint32_t bar1) {
+  const uint32_t idesc = F8 ? (mn_major ? make_idesc_e4m3(T, T / 2, 0, 1) : make_idesc_e4m3(T, T / 2, 0, 0))
+                            : (mn_major ? make_idesc_bf16(T, T / 2, 0, 1) : make_idesc_bf16(T, T / 2, 0, 0));
 #pragma unroll
-  for (int kk = 0; kk < T / (F8 ? 32 : 16); ++kk) {
-    const uint64_t db = mn_major ? desc_mnmajor<F8>(buf, kk) : desc_kmajor(buf, kk);
-    if (F8) umma_f8_ts_pair(acc, opa + 8 * kk, db, idesc, kk ? 1u : 0u);
-    else umma_bf16_ts_pair(acc, opa + 8 * kk, db, idesc, kk ? 1u : 0u);
+  for (int hb = 0; hb < 2; ++hb) {
+    // K-major B: 64 rows of 128 B further on; MN-major B: the next 64 columns (bf16: the second atom; e4m3: 64 B on)
+    const uint32_t bh = buf + (mn_major ? (F8 ? 64u : kAtomBytes) : 64u * 128u) * hb;
+#pragma unroll
+    for (int kk = 0; kk < T / (F8 ? 32 : 16); ++kk) {
+      const uint64_t db = mn_major ? desc_mnmajor<F8>(bh, kk) : desc_kmajor(bh, kk);
+      if (F8) umma_f8_ts_pair(acc + 128 * hb, opa + 8 * kk, db, idesc, kk ? 1u : 0u);
+      else umma_bf16_ts_pair(acc + 128 * hb, opa + 8 * kk, db, idesc, kk ? 1u : 0u);
+    }
+    umma_commit_pair(hb ? bar1 : bar0, (uint16_t)3);
   }
-  umma_commit_pair(bar, (uint16_t)3);
 }
 
 template <bool F8>
@@ -117,34 +132,45 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   const int R = (int)rank * kRows + t; // row of the tile
   const bool lead = (tid == 0);
   const bool step_mode = (mode == MODE_STEP);
-  // diagonal element (R, R): column quarter R >> 6, 16-column chunk (R & 63) >> 4 of it; bf16: packed word (R & 15) >> 1,
-  // half R & 1; e4m3: packed word (R & 15) >> 2, byte R & 3
-  const bool own = (q4 == (int)(2 * rank) + (wq >> 1));            // warp-uniform
-  const int dq = (t & 63) >> 4, dword = F8 ? (t & 15) >> 2 : (t & 15) >> 1;
+  // Column ownership: thread (t, q4) owns the 32-column half s2 = q4 & 1 of the two adjacent global 64-column blocks
+  // 2 bp and 2 bp + 1, bp = q4 >> 1, as four 16-column pieces q = 2 hb + j (block 2 bp + hb, chunk j).  Block 2 bp + hb
+  // lies in half hb of the accumulator (issue_pair), so every thread has half of its work in each N-half of a product.
+  const int s2 = q4 & 1, bp = q4 >> 1;
+  // diagonal element (R, R), R = 128 rank + t: block 2 rank + (t >> 6), inner half (t >> 5) & 1, chunk (t >> 4) & 1; bf16:
+  // packed word (R & 15) >> 1, half R & 1; e4m3: packed word (R & 15) >> 2, byte R & 3
+  const bool own = (q4 == (int)(2 * rank) + (wq & 1));             // warp-uniform
+  const int dq = 2 * (wq >> 1) + ((lane >> 4) & 1), dword = F8 ? (t & 15) >> 2 : (t & 15) >> 1;
   const uint32_t dshift = F8 ? (uint32_t)(t & 3) * 8u : (uint32_t)(t & 1) * 16u;
   const uint32_t dkeep = ~((F8 ? 0xffu : 0xffffu) << dshift);
 
   const uint32_t XB = smem0, OB = XB + kBufBytes, ST = OB + kBufBytes;
-  const uint32_t rowoff = (uint32_t)q4 * kBlkBytes + (uint32_t)t * 128u + ((uint32_t)(t & 7) << 4);
-  const uint32_t xrow = XB + rowoff, orow = OB + rowoff, srow = ST + rowoff;   // bf16 rows (operands, and staging of G / M / W)
-  // e4m3 operand rows (first 32 KB of XB / OB): K-span block q4 >> 1, this thread's 64 bytes = chunks 4(q4&1)..+3
-  const uint32_t row8 = (uint32_t)(q4 >> 1) * kBlkBytes + (uint32_t)t * 128u + ((uint32_t)((4 * (q4 & 1)) ^ (t & 7)) << 4);
-  const uint32_t xrow8 = XB + row8, orow8 = OB + row8;
-  // this thread's 64 columns of row R in the MN-major (column-split) copy of Xb, which lives in the staging
-  // buffer ST during the steps: CTA q4 >> 1, atom q4 & 1, K-row R
-  // (e4m3: one 128-byte span per K-row, this thread's 64 bytes = chunks 4(q4&1)..+3 of it)
-  const uint32_t xt_local = F8 ? ST + (uint32_t)R * 128u + ((uint32_t)((4 * (q4 & 1)) ^ (R & 7)) << 4)
-                               : ST + (uint32_t)(q4 & 1) * kAtomBytes + (uint32_t)R * 128u + ((uint32_t)(R & 7) << 4);
-  const bool xt_is_local = ((uint32_t)(q4 >> 1) == rank);              // warp-uniform
-  const uint32_t xt_row = xt_is_local ? xt_local : mapa_shared(xt_local, (uint32_t)(q4 >> 1));
-  const uint32_t mma_bar = smem_u32(&ctrl->mma_bar);
+  // bf16 rows (operands, and staging of G / M / W): 8-column chunk c = 4 hb + 2 j + e of this thread's 64 columns is
+  // 16-byte chunk (4 s2 + (c & 3)) ^ (t & 7) of row t of 64-column block 2 bp + (c >> 2)
+  const uint32_t base16 = (uint32_t)(2 * bp) * kBlkBytes + (uint32_t)t * 128u + ((((uint32_t)(4 * s2)) ^ (uint32_t)(t & 7)) << 4);
+  auto addr16 = [&](uint32_t buf, int c) { return buf + (base16 ^ ((uint32_t)(c & 3) << 4)) + (uint32_t)(c >> 2) * kBlkBytes; };
+  // e4m3 operand rows (first 32 KB of XB / OB): 128-byte block bp of row t, piece q = 16 bytes = chunk 4 hb + 2 s2 + j
+  const uint32_t base8 = (uint32_t)bp * kBlkBytes + (uint32_t)t * 128u + ((((uint32_t)(2 * s2)) ^ (uint32_t)(t & 7)) << 4);
+  auto addr8 = [&](uint32_t buf, int q) { return buf + (base8 ^ ((uint32_t)(4 * (q >> 1) + (q & 1)) << 4)); };
+  // this thread's columns of row R in the MN-major (column-split) copy of Xb, which lives in the staging buffer ST
+  // during the steps: both of its blocks belong to CTA bp; K-row R; bf16: atom hb, chunks 4 s2 + 2 j + e of the 128-byte
+  // row; e4m3: one 128-byte span per K-row, chunk 4 hb + 2 s2 + j
+  const uint32_t xt_local = F8 ? ST + (uint32_t)R * 128u + ((uint32_t)((2 * s2) ^ (R & 7)) << 4)
+                               : ST + (uint32_t)R * 128u + ((uint32_t)((4 * s2) ^ (R & 7)) << 4);
+  const bool xt_is_local = ((uint32_t)bp == rank);                     // warp-uniform
+  const uint32_t xt_row = xt_is_local ? xt_local : mapa_shared(xt_local, (uint32_t)bp);
+  auto xt_addr = [&](int q, int e) {
+    return F8 ? (xt_row ^ ((uint32_t)(4 * (q >> 1) + (q & 1)) << 4))
+              : (xt_row ^ ((uint32_t)(2 * (q & 1) + e) << 4)) + (uint32_t)(q >> 1) * kAtomBytes;
+  };
+  const uint32_t mma_bar0 = smem_u32(&ctrl->mma_bar[0]), mma_bar1 = smem_u32(&ctrl->mma_bar[1]);
   const uint32_t ready_bar = smem_u32(&ctrl->ready_bar);
   const uint32_t ready_bar_leader = mapa_shared(ready_bar, 0);
   const uint32_t ld_bar = smem_u32(&ctrl->ld_bar);
   const uint32_t w_bar = smem_u32(&ctrl->w_bar);
 
   if (tid == 0) {
-    mbar_init(mma_bar, 1);
+    mbar_init(mma_bar0, 1);
+    mbar_init(mma_bar1, 1);
     mbar_init(ready_bar, 2);
     mbar_init(ld_bar, 2);   // arrive.expect_tx at issue + "staging buffer is free" arrive of the lead thread
     mbar_init(w_bar, 1);
@@ -157,11 +183,18 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
   tc_fence_after_sync();
   const uint32_t tmem_base = ctrl->tmem_base;
   const uint32_t lane_off = (uint32_t)(wq * 32) << 16;
-  const uint32_t acc_t = tmem_base + lane_off + kAccCol + 64u * q4;   // this thread's 64 accumulator columns
-  const uint32_t opa_t = tmem_base + lane_off + kOpaCol + (F8 ? 16u : 32u) * q4;   // this thread's 32 (e4m3: 16) packed operand columns
+  // piece q = 2 hb + j: accumulator columns 128 hb + 64 bp + 32 s2 + 16 j; operand columns of the global chunk
+  // 8 bp + 4 hb + 2 s2 + j (8 packed columns per chunk, e4m3: 4)
+  const uint32_t acc_t = tmem_base + lane_off + kAccCol + 64u * bp + 32u * s2;
+  const uint32_t opa_t = tmem_base + lane_off + kOpaCol + (F8 ? 4u : 8u) * (8u * bp + 2u * s2);
+  auto acc_q = [&](int q) { return acc_t + 128u * (q >> 1) + 16u * (q & 1); };
+  auto opa_q = [&](int q) { return opa_t + (F8 ? 4u : 8u) * (4u * (q >> 1) + (q & 1)); };
   const uint32_t ACCd = tmem_base + kAccCol, OPAd = tmem_base + kOpaCol;
 
   uint32_t ph_mma = 0, ph_ld = 0, ph_w = 0, ph_ready = 0;
+  // The A operand is double-buffered in tensor memory (columns 256.. / 384..): an epilogue that starts on the first
+  // N-half writes the NEXT product's operand while the second half still reads the current one.
+  uint32_t opw = 0;            // column offset (0 / 128) of the operand buffer being written
   const float qs = sqrtf(sqrtf(hp.c));         // state Xh = c^(1/4) X, see kernels_tc128.cu
   const float beta_h = hp.b / sqrtf(hp.c);
 
@@ -182,17 +215,18 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         if (rank == 0) {
           mbar_wait_cluster(ready_bar, ph_ready);
           tc_fence_after_sync();
-          issue_pair<F8>(ACCd, OPAd, which == 1 ? OB : which == 2 ? XB : ST, which == 3, mma_bar);
+          issue_pair<F8>(ACCd, OPAd + opw, which == 1 ? OB : which == 2 ? XB : ST, which == 3, mma_bar0, mma_bar1);
         }
       }
       __syncwarp();
     }
     ph_ready ^= 1;
+    opw ^= 128u;               // the next epilogue writes the other operand buffer
   };
-  auto wait_mma = [&]() {   // one warp polls, the others sleep on a hardware barrier
-    if (warp == 0) mbar_wait(mma_bar, ph_mma);
-    named_bar_sync(1, kThreads);
-    ph_mma ^= 1;
+  // N-half hb of the current product is complete (ph_mma flips once per product, after half 1)
+  auto wait_mma = [&](int hb) {
+    mbar_wait_parked(hb ? mma_bar1 : mma_bar0, ph_mma);
+    if (hb) ph_mma ^= 1;
     tc_fence_after_sync();
   };
 
@@ -209,43 +243,43 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         uint32_t x4[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) x4[j] = cvt_e4m3x4(mul2(xs[8 * q + 2 * j], sx2), mul2(xs[8 * q + 2 * j + 1], sx2));
-        if (xt_is_local) sts128(chunk_addr(xt_row, q), make_uint4(x4[0], x4[1], x4[2], x4[3]));
-        else st_cluster_v4(chunk_addr(xt_row, q), make_uint4(x4[0], x4[1], x4[2], x4[3]));
+        if (xt_is_local) sts128(xt_addr(q, 0), make_uint4(x4[0], x4[1], x4[2], x4[3]));
+        else st_cluster_v4(xt_addr(q, 0), make_uint4(x4[0], x4[1], x4[2], x4[3]));
       } else {
         uint32_t x8[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) x8[j] = cvt_bf16x2(xs[8 * q + j]);
         if (xt_is_local) {
-          sts128(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
-          sts128(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
+          sts128(xt_addr(q, 0), make_uint4(x8[0], x8[1], x8[2], x8[3]));
+          sts128(xt_addr(q, 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
         } else {
-          st_cluster_v4(chunk_addr(xt_row, 2 * q), make_uint4(x8[0], x8[1], x8[2], x8[3]));
-          st_cluster_v4(chunk_addr(xt_row, 2 * q + 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
+          st_cluster_v4(xt_addr(q, 0), make_uint4(x8[0], x8[1], x8[2], x8[3]));
+          st_cluster_v4(xt_addr(q, 1), make_uint4(x8[4], x8[5], x8[6], x8[7]));
         }
       }
     }
   };
   // 16 columns (chunk q of this thread's 64) of the next A operand: rounded to the operand format (e4m3: scaled by
   // `scale` first), the diagonal element replaced by dval when this thread owns it (diag), written to this thread's
-  // TMEM operand columns and, if row16 is given, to the K-major shared-memory operand (bf16 row row16 / e4m3 row row8).
-  auto emit_operand = [&](const f2 (&v)[8], f2 scale, int q, bool diag, uint32_t dval, uint32_t row16, uint32_t row8) {
+  // TMEM operand columns and, if buf is given (XB / OB), to the K-major shared-memory operand in that buffer.
+  auto emit_operand = [&](const f2 (&v)[8], f2 scale, int q, bool diag, uint32_t dval, uint32_t buf) {
     if (F8) {
       uint32_t p[4];
 #pragma unroll
       for (int j = 0; j < 4; ++j) p[j] = cvt_e4m3x4(mul2(v[2 * j], scale), mul2(v[2 * j + 1], scale));
       if (diag) set_one4(p, dq == q ? dword : 4, dkeep, dval);
-      if (row8) sts128(chunk_addr(row8, q), make_uint4(p[0], p[1], p[2], p[3]));
-      tmem_st4(opa_t + 4 * q, p);
+      if (buf) sts128(addr8(buf, q), make_uint4(p[0], p[1], p[2], p[3]));
+      tmem_st4(opa_q(q) + opw, p);
     } else {
       uint32_t p[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) p[j] = cvt_bf16x2(v[j]);
       if (diag) set_one(p, dq == q ? dword : 8, dkeep, dval);
-      if (row16) {
-        sts128(chunk_addr(row16, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
-        sts128(chunk_addr(row16, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
+      if (buf) {
+        sts128(addr16(buf, 2 * q), make_uint4(p[0], p[1], p[2], p[3]));
+        sts128(addr16(buf, 2 * q + 1), make_uint4(p[4], p[5], p[6], p[7]));
       }
-      tmem_st8(opa_t + 8 * q, p);
+      tmem_st8(opa_q(q) + opw, p);
     }
   };
   auto acc_pairs = [](const uint32_t (&c)[16], f2 (&v)[8]) {
@@ -295,10 +329,10 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     const f2 beta2 = pk2(hp.beta, hp.beta);
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
-      const uint4 gv = lds128(chunk_addr(orow, c));
+      const uint4 gv = lds128(addr16(OB, c));
       const uint32_t gw[4] = {gv.x, gv.y, gv.z, gv.w};
       if (step_mode) {
-        const uint4 mv = lds128(chunk_addr(xrow, c));
+        const uint4 mv = lds128(addr16(XB, c));
         const uint32_t mw[4] = {mv.x, mv.y, mv.z, mv.w};
         uint32_t mo[4];
 #pragma unroll
@@ -310,7 +344,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           ss2 = fma2(h2, h2, ss2);
           xs[4 * c + e] = h2;
         }
-        sts128(chunk_addr(xrow, c), make_uint4(mo[0], mo[1], mo[2], mo[3]));   // M' in place, over this thread's M
+        sts128(addr16(XB, c), make_uint4(mo[0], mo[1], mo[2], mo[3]));   // M' in place, over this thread's M
       } else {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
@@ -363,7 +397,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         f2 v[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) v[j] = xs[8 * q + j] = mul2(xs[8 * q + j], inv2);
-        emit_operand(v, sx2, q, false, 0u, orow, orow8);   // Xb lives in OB (G is consumed), Ot in XB: see the M' store above
+        emit_operand(v, sx2, q, false, 0u, OB);   // Xb lives in OB (G is consumed), Ot in XB: see the M' store above
       }
     }
     TR();   // prologue compute done
@@ -378,9 +412,12 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
     for (int k = 0; k < hp.K; ++k) {
       const bool last = (k + 1 == hp.K);
       // ---- E1: ACC = rows of Ah
-      if (lead && k == 0 && step_mode) tma_wait_group_read0();   // M' has left XB (long ago): Ot may be written into it
-      wait_mma();
-      TR();   // MMA1 done
+      if (k == 0 && step_mode) {                                 // M' has left XB (long ago): Ot may be written into it
+        if (lead) tma_wait_group_read0();
+        __syncthreads();
+      }
+      wait_mma(0);
+      TR();   // MMA1 done (first half)
       {
         // Ot = offdiag(Ah) + diag(d + beta/2), rounded to bf16: offdiag(Ot Ot^T) = offdiag(beta Ah + Ah^2)
         // (e4m3: ACC = s_X^2 Ah; operand scale s_O: Ot s_O = ACC s_O / s_X^2)
@@ -390,11 +427,11 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
         const f2 k1 = pk2(kSO / (kSX * kSX), kSO / (kSX * kSX));
         f2 Sa = pk2(0.f, 0.f), Sb = Sa;
         uint32_t r[2][16];
-        tmem_ld16(acc_t, r[0]);
+        tmem_ld16(acc_q(0), r[0]);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           tmem_wait_ld();
-          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          if (q != 1 && q < 3) tmem_ld16(acc_q(q + 1), r[(q + 1) & 1]);
           uint32_t(&c)[16] = r[q & 1];
 #pragma unroll
           for (int j = 0; j < 4; ++j) {
@@ -404,7 +441,11 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
           }
           f2 v[8];
           acc_pairs(c, v);
-          emit_operand(v, k1, q, own, dval, xrow, xrow8);
+          emit_operand(v, k1, q, own, dval, XB);
+          if (q == 1) {                              // pieces 2, 3 live in the second N-half
+            wait_mma(1);
+            tmem_ld16(acc_q(2), r[0]);
+          }
         }
         float s0, s1;
         upk2(add2(Sa, Sb), s0, s1);
@@ -418,18 +459,22 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       const float si = hp.a + fmaf(beta_h, di, (ctrl->spart[0][t] + ctrl->spart[1][t]) + (ctrl->spart[2][t] + ctrl->spart[3][t]));
 
       // ---- E2: ACC = rows of B (off-diagonal)
-      wait_mma();
-      TR();   // MMA2 done
+      wait_mma(0);
+      TR();   // MMA2 done (first half)
       {
         uint32_t r[2][16];
-        tmem_ld16(acc_t, r[0]);
+        tmem_ld16(acc_q(0), r[0]);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           tmem_wait_ld();
-          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          if (q != 1 && q < 3) tmem_ld16(acc_q(q + 1), r[(q + 1) & 1]);
           f2 v[8];
           acc_pairs(r[q & 1], v);
-          emit_operand(v, pk2(kSB / (kSO * kSO), kSB / (kSO * kSO)), q, own, 0u, 0u, 0u);   // e4m3: ACC = s_O^2 B; operand Bb s_B
+          emit_operand(v, pk2(kSB / (kSO * kSO), kSB / (kSO * kSO)), q, own, 0u, 0u);   // e4m3: ACC = s_O^2 B; operand Bb s_B
+          if (q == 1) {
+            wait_mma(1);
+            tmem_ld16(acc_q(2), r[0]);
+          }
         }
       }
       TR();   // E2 loop done
@@ -437,27 +482,29 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       TR();   // MMA3 issued
 
       // ---- E3: Xh = (a + B_RR) Xh + offdiag(B) Xh
-      wait_mma();
-      TR();   // MMA3 done
-      if (last && lead && step_mode) {                       // ST is free (every pair MMA has completed): fetch W into
-        mbar_arrive_expect_tx(w_bar, kBufBytes);             // it - FIRST, phase F needs it long before P needs G, M
+      wait_mma(0);
+      TR();   // MMA3 done (first half)
+      auto after_last_mma = [&]() {
+        if (last && lead && step_mode) {                     // ST is free (every pair MMA has completed): fetch W into
+          mbar_arrive_expect_tx(w_bar, kBufBytes);           // it - FIRST, phase F needs it long before P needs G, M
 #pragma unroll
-        for (int j = 0; j < 4; ++j) tma_load_2d(ST + j * kBlkBytes, map_w, x0 + 64 * j, y0, w_bar);
-        w_issued = true;
-      }
-      if (last && nxt < n_items) {                           // ... and so are XB and OB: the next tile's G and M
-        if (lead) issue_gm(nxt);
-        prefetched = true;
-      }
+          for (int j = 0; j < 4; ++j) tma_load_2d(ST + j * kBlkBytes, map_w, x0 + 64 * j, y0, w_bar);
+          w_issued = true;
+        }
+        if (last && nxt < n_items) {                         // ... and so are XB and OB: the next tile's G and M
+          if (lead) issue_gm(nxt);
+          prefetched = true;
+        }
+      };
       {
         const f2 si2 = pk2(si, si), k3 = pk2(1.f / (kSB * kSX), 1.f / (kSB * kSX)), sx2 = pk2(kSX, kSX);
         f2 Da = pk2(0.f, 0.f), Db = Da;
         uint32_t r[2][16];
-        tmem_ld16(acc_t, r[0]);
+        tmem_ld16(acc_q(0), r[0]);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           tmem_wait_ld();
-          if (q < 3) tmem_ld16(acc_t + 16 * (q + 1), r[(q + 1) & 1]);
+          if (q != 1 && q < 3) tmem_ld16(acc_q(q + 1), r[(q + 1) & 1]);
           uint32_t(&c)[16] = r[q & 1];
 #pragma unroll
           for (int j = 0; j < 8; ++j)
@@ -472,7 +519,12 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
             f2 v[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) v[j] = xs[8 * q + j];
-            emit_operand(v, sx2, q, false, 0u, orow, orow8);
+            emit_operand(v, sx2, q, false, 0u, OB);
+          }
+          if (q == 1) {
+            wait_mma(1);
+            after_last_mma();
+            tmem_ld16(acc_q(2), r[0]);
           }
         }
         if (!last) {
@@ -516,7 +568,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
       for (int c = 0; c < 8; ++c) {
         uint32_t p[4];
         if (step_mode) {
-          const uint4 wv = lds128(chunk_addr(srow, c));
+          const uint4 wv = lds128(addr16(ST, c));
           const uint32_t ww[4] = {wv.x, wv.y, wv.z, wv.w};
 #pragma unroll
           for (int e = 0; e < 4; ++e)
@@ -525,7 +577,7 @@ himuon_tc256_kernel(const LayerDev* __restrict__ layers, const CUtensorMap* __re
 #pragma unroll
           for (int e = 0; e < 4; ++e) p[e] = cvt_bf16x2(mul2(step2, xs[4 * c + e]));
         }
-        sts128(chunk_addr(srow, c), make_uint4(p[0], p[1], p[2], p[3]));
+        sts128(addr16(ST, c), make_uint4(p[0], p[1], p[2], p[3]));
       }
     }
     fence_proxy_async_smem();

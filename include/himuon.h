@@ -60,7 +60,7 @@ typedef enum { HIMUON_F32 = 0, HIMUON_BF16 = 1 } himuon_dtype;
  *            T = 256      tcgen05 cta_group::2, one tile per CTA pair      (same)
  *            T = 512, the full-matrix branch T >= max(H,W) > 256 and rectangular tiles: large-tile path - every
  *                         product of a Newton-Schulz step is one launch of a hand-written persistent tcgen05 GEMM
- *                         (bf16 operands, fp32 accumulation, fp32 iterate) with the step's elementwise work fused
+ *                         (bf16 operands, fp32 accumulation, the iterate as a bf16 hi + lo pair) with the step's elementwise work fused
  *                         into its epilogue; tiles staged in sub-batches inside the caller's workspace
  *                         (himuon_plan_info reports the bytes)
  *          a bf16 matrix whose width is not a multiple of 8 is served by the fp32 kernel at T = 64, 128 and by

@@ -1,10 +1,11 @@
 """One tiny ragged Algorithm-4.1 step per kernel of the library, each checked against the float64 oracle.
 
 Small enough to run under `compute-sanitizer` (racecheck / synccheck / memcheck): the
-hand-written mbarrier / TMEM / TMA pipelines are exactly the kind of code those tools exist for.  The summaries of
-those runs are under profiles/ (r2_sanitizer_*.txt), each naming its command:
+hand-written mbarrier / TMEM / TMA pipelines are exactly the kind of code those tools exist for.  The command
 
     compute-sanitizer --tool <tool> python -m pytest tests/test_gpu_tiny_all_kernels.py -m gpu -q
+
+is refused by this GPU pool (profiles/r2_sanitizer.md says what was asked and what stands in for it).
 """
 import pytest
 import torch
@@ -46,11 +47,7 @@ def test_tiny_ragged_step(name, dtype, path, T, shape, tol):
     plan.step(hp)          # a second step reuses every buffer, barrier phase and prefetch of the persistent kernels
     torch.cuda.synchronize()
     plan.destroy()
-    # oracle: the same two steps
-    ohp = PU.oracle_hp(hp)
-    W1, M1, _ = PU.O.step(PU.f64(W0), PU.f64(G), PU.f64(M0), ohp, T)
     bf = dtype == torch.bfloat16
-    r = (lambda x: I.bf16_round_f64(x)) if bf else (lambda x: x.astype("float32").astype("float64"))
     # second step from the GPU's own stored state of the first (the stored M', W' are what it reads back)
     plan1 = hm.Plan.from_tensors([W0.to(DEV)], [Gd], [M0.to(DEV)], T, path=path).bind()
     plan1.step(hp)

@@ -173,7 +173,7 @@ __device__ __forceinline__ uint4 pack8(const float (&f)[8]) {
   return make_uint4(pack_bf16(f[0], f[1]), pack_bf16(f[2], f[3]), pack_bf16(f[4], f[5]), pack_bf16(f[6], f[7]));
 }
 
-// grid (kPrepBlocks, nb), one warp per row of the SCRATCH layout (rp x ldx, coalesced writes); element (i, j) of the
+// grid (kPrepBlocks, nb) (big tiles: more blocks, ssq == nullptr), one warp per row of the SCRATCH layout (rp x ldx, coalesced writes); element (i, j) of the
 // iterate is element (i, j) of the tile, or (j, i) when transposed.  Untransposed tiles whose rows are 16-byte aligned
 // take the wide path: a lane owns 8 consecutive columns of a BN-column slot, both loads of a slot pair are issued
 // before the first store (the stores to M could alias the loads of G for all the compiler knows).
@@ -189,7 +189,7 @@ lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items,
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   float ss = 0.f;
   if (!g.transposed && tile_vec8(t, step_mode != 0)) {
-    for (int i = blockIdx.x * (kEwThreads / 32) + warp; i < g.rp; i += kPrepBlocks * (kEwThreads / 32)) {
+    for (int i = blockIdx.x * (kEwThreads / 32) + warp; i < g.rp; i += (int)gridDim.x * (kEwThreads / 32)) {
       const bool row_ok = i < t.h;
       for (int slot0 = 0; slot0 < g.ntx; slot0 += 2) {
         uint4 gv[2], mv[2];
@@ -240,7 +240,7 @@ lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items,
       }
     }
   } else {
-    for (int i = blockIdx.x * (kEwThreads / 32) + warp; i < g.rp; i += kPrepBlocks * (kEwThreads / 32)) {
+    for (int i = blockIdx.x * (kEwThreads / 32) + warp; i < g.rp; i += (int)gridDim.x * (kEwThreads / 32)) {
       for (int slot = 0; slot < g.ntx; ++slot) {        // d partial per BN-column slot, as the E3 epilogue writes them
         float dd = 0.f;
         const int j1 = min((slot + 1) * BN, g.ldx);
@@ -272,7 +272,7 @@ lt_prep(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items,
   __shared__ float red[kEwThreads / 32];
   if (lane == 0) red[warp] = ss;
   __syncthreads();
-  if (threadIdx.x == 0) {
+  if (threadIdx.x == 0 && ssq) {      // (big tiles run on a wider grid and take the sum from the d partials: lt_ssq_from_d)
     float tot = 0.f;
 #pragma unroll
     for (int i = 0; i < kEwThreads / 32; ++i) tot += red[i];
@@ -294,7 +294,7 @@ lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ item
   if (!g.transposed && tile_vec8(t, false)) {
     // wide path: a thread owns 8 consecutive columns of a row; two such pieces in flight per thread
     const int w8 = t.w_ / 8;
-    const long long n8 = (long long)t.h * w8, stride = (long long)kPrepBlocks * kEwThreads;
+    const long long n8 = (long long)t.h * w8, stride = (long long)gridDim.x * kEwThreads;
     for (long long e0 = (long long)blockIdx.x * kEwThreads + threadIdx.x; e0 < n8; e0 += 2 * stride) {
       uint4 xh[2], xl[2];
       uint4 wv[2];
@@ -335,13 +335,175 @@ lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ item
     return;
   }
   const long long n = (long long)t.h * t.w_;
-  for (long long e = (long long)blockIdx.x * kEwThreads + threadIdx.x; e < n; e += (long long)kPrepBlocks * kEwThreads) {
+  for (long long e = (long long)blockIdx.x * kEwThreads + threadIdx.x; e < n; e += (long long)gridDim.x * kEwThreads) {
     const int r = (int)(e / t.w_), c = (int)(e - (long long)r * t.w_);
     const long long at = g.transposed ? (long long)c * g.ldx + r : (long long)r * g.ldx + c;
     const float x = __bfloat162float(Xh[at]) + __bfloat162float(Xl[at]);
     __nv_bfloat16* p = t.w + (long long)r * t.ld_w + c;
     *p = __float2bfloat16_rn(step_mode ? fmaf(keep, __bfloat162float(*p), stepsz * x) : stepsz * x);
   }
+}
+
+// ---- fused ends of BIG tiles (the full-matrix branch, tiles of >= 1 M elements) ----------------------------------------
+// With one tile (or a few) per sub-batch the kPrepBlocks x nb grid of lt_prep / lt_update is a fraction of the GPU, and the
+// scalar path of a TRANSPOSED tile touches one 2-byte element per lane and row (measured on a 14336 x 4096 matrix: 6.3 ms
+// of lt_prep + 4.3 ms of lt_update beside 4.2 ms for the fifteen GEMMs).  Big tiles therefore run lt_prep / lt_update on a
+// grid sized by the tile, transposed tiles go through the two kernels below (64 x 64 patches transposed in shared
+// memory: every global access is a row segment in BOTH layouts), and the sum of squares of the tile comes from the d
+// partials in one fixed order (lt_ssq_from_d).
+constexpr int kTP = 64;                   // patch edge
+
+// 16 consecutive bf16 -> fp32 (the first nv of them; the rest read as zero) and back; 16-byte accesses when `vec`
+__device__ __forceinline__ void load16(const __nv_bfloat16* p, int nv, bool vec, float (&f)[16]) {
+  if (vec && nv == 16) {
+    float a[8], b[8];
+    unpack8(*reinterpret_cast<const uint4*>(p), a);
+    unpack8(*reinterpret_cast<const uint4*>(p + 8), b);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { f[k] = a[k]; f[8 + k] = b[k]; }
+  } else {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) f[k] = k < nv ? __bfloat162float(p[k]) : 0.f;
+  }
+}
+__device__ __forceinline__ void store16(__nv_bfloat16* p, int nv, bool vec, const float (&f)[16]) {
+  if (vec && nv == 16) {
+    const float a[8] = {f[0], f[1], f[2], f[3], f[4], f[5], f[6], f[7]};
+    const float b[8] = {f[8], f[9], f[10], f[11], f[12], f[13], f[14], f[15]};
+    *reinterpret_cast<uint4*>(p) = pack8(a);
+    *reinterpret_cast<uint4*>(p + 8) = pack8(b);
+  } else {
+#pragma unroll
+    for (int k = 0; k < 16; ++k)
+      if (k < nv) p[k] = __float2bfloat16_rn(f[k]);
+  }
+}
+
+// lt_prep for transposed tiles: iterate (i, j) = tile (j, i).  grid (ceil(rp / 64), ntx, nb), 256 threads; a block owns
+// iterate rows C0 .. C0 + 63 (tile columns) and the iterate columns of d-partial slot blockIdx.y (tile rows), 64 at a time.
+__global__ void __launch_bounds__(kEwThreads)
+lt_prep_t(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, LtGeom g, int whole,
+          __nv_bfloat16* __restrict__ xlo, __nv_bfloat16* __restrict__ xb, long long sxb, float* __restrict__ d0, long long sd,
+          int step_mode, float beta, int nesterov) {
+  const int b = blockIdx.z;
+  const TileRef t = tile_ref(layers, items, b, g.Th, g.Tw, whole);
+  __nv_bfloat16* Xl = xlo + (long long)b * sxb;
+  __nv_bfloat16* Xb = xb + (long long)b * sxb;
+  float* D = d0 + (long long)b * sd;
+  const int slot = blockIdx.y, C0 = blockIdx.x * kTP;
+  const int rr = threadIdx.x >> 2, seg = threadIdx.x & 3;
+  const bool vec = tile_vec8(t, step_mode != 0);
+  __shared__ float xs[kTP][kTP + 1];
+  float dd = 0.f;                          // this thread's share of sum_j x_ij^2, i = C0 + rr, j in the slot
+  const int jend = min((slot + 1) * BN, g.ldx);
+  for (int R0 = slot * BN; R0 < jend; R0 += kTP) {
+    {   // tile row R0 + rr, tile columns C0 + 16 seg .. + 15: momentum in the tile's own layout
+      const int r = R0 + rr, c0 = C0 + 16 * seg;
+      float x[16];
+#pragma unroll
+      for (int k = 0; k < 16; ++k) x[k] = 0.f;                               // outside the tile: B_T zero padding
+      if (r < t.h && c0 < t.w_) {
+        const int nv = min(16, t.w_ - c0);
+        load16(t.g + (long long)r * t.ld_g + c0, nv, vec, x);
+        if (step_mode) {
+          float m[16];
+          __nv_bfloat16* pm = t.m + (long long)r * t.ld_m + c0;
+          load16(pm, nv, vec, m);
+#pragma unroll
+          for (int k = 0; k < 16; ++k) m[k] = fmaf(beta, m[k], x[k]);
+          store16(pm, nv, vec, m);
+#pragma unroll
+          for (int k = 0; k < 16; ++k) x[k] = k < nv ? (nesterov ? fmaf(beta, m[k], x[k]) : m[k]) : 0.f;
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 16; ++k) xs[16 * seg + k][rr] = x[k];
+    }
+    __syncthreads();
+    {   // iterate row C0 + rr, iterate columns R0 + 16 seg .. + 15 (ldx is a multiple of 64: whole segments)
+      const int i = C0 + rr, j0 = R0 + 16 * seg;
+      if (i < g.rp) {
+        float h[16], l[16];
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+          const float x = xs[rr][16 * seg + k];
+          h[k] = __bfloat162float(__float2bfloat16_rn(x));
+          l[k] = x - h[k];
+          dd = fmaf(x, x, dd);
+        }
+        store16(Xb + (long long)i * g.ldx + j0, 16, true, h);
+        store16(Xl + (long long)i * g.ldx + j0, 16, true, l);
+      }
+    }
+    __syncthreads();
+  }
+  dd += __shfl_xor_sync(0xffffffffu, dd, 1);
+  dd += __shfl_xor_sync(0xffffffffu, dd, 2);
+  if (seg == 0 && C0 + rr < g.rp) D[(long long)slot * g.rp + C0 + rr] = dd;
+}
+
+// lt_update for transposed tiles.  grid (ceil(rp / 64), ceil(np / 64), nb), 256 threads.
+__global__ void __launch_bounds__(kEwThreads)
+lt_update_t(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ items, LtGeom g, int whole,
+            const __nv_bfloat16* __restrict__ xhi, const __nv_bfloat16* __restrict__ xlo, long long sxb, int step_mode, float keep,
+            float lr_scale, float unq, const float* __restrict__ ssq, float eps, float qs) {
+  const int b = blockIdx.z;
+  const TileRef t = tile_ref(layers, items, b, g.Th, g.Tw, whole);
+  const __nv_bfloat16* Xh = xhi + (long long)b * sxb;
+  const __nv_bfloat16* Xl = xlo + (long long)b * sxb;
+  const float sig = ssq ? tile_sigma(ssq, b, eps, qs) : 1.f;      // K = 0: the iterate is still the raw Ghat
+  const float stepsz = (step_mode ? lr_scale * t.tau_base * unq : unq) * sig;
+  const int C0 = blockIdx.x * kTP, R0 = blockIdx.y * kTP;
+  const int rr = threadIdx.x >> 2, seg = threadIdx.x & 3;
+  __shared__ float xs[kTP][kTP + 1];
+  {   // iterate row C0 + rr, iterate columns R0 + 16 seg .. + 15
+    const int i = C0 + rr, j0 = R0 + 16 * seg;
+    float h[16], l[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) h[k] = l[k] = 0.f;
+    if (i < g.rp && j0 < g.ldx) {
+      load16(Xh + (long long)i * g.ldx + j0, 16, true, h);
+      load16(Xl + (long long)i * g.ldx + j0, 16, true, l);
+    }
+#pragma unroll
+    for (int k = 0; k < 16; ++k) xs[rr][16 * seg + k] = h[k] + l[k];
+  }
+  __syncthreads();
+  {   // tile row R0 + rr, tile columns C0 + 16 seg .. + 15
+    const int r = R0 + rr, c0 = C0 + 16 * seg;
+    if (r < t.h && c0 < t.w_) {
+      const int nv = min(16, t.w_ - c0);
+      const bool vec = tile_vec8(t, false);
+      __nv_bfloat16* pw = t.w + (long long)r * t.ld_w + c0;
+      float o[16];
+      if (step_mode) {
+        load16(pw, nv, vec, o);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) o[k] = fmaf(keep, o[k], stepsz * xs[16 * seg + k][rr]);
+      } else {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) o[k] = stepsz * xs[16 * seg + k][rr];
+      }
+      store16(pw, nv, vec, o);
+    }
+  }
+}
+
+// ||Ghat||_F^2 of every tile from its d partials (row sums of squares), in one fixed order -> the slot layout tile_sigma reads
+__global__ void __launch_bounds__(1024)
+lt_ssq_from_d(const float* __restrict__ d0, long long sd, int n, float* __restrict__ ssq) {
+  const int b = blockIdx.x;
+  const float* D = d0 + (long long)b * sd;
+  __shared__ float red[1024];
+  float s = 0.f;
+  for (int e = threadIdx.x; e < n; e += 1024) s += D[e];
+  red[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x < kPrepBlocks) ssq[(long long)b * kPrepBlocks + threadIdx.x] = threadIdx.x == 0 ? red[0] : 0.f;
 }
 
 // ---- the GEMM --------------------------------------------------------------------------------------------------
@@ -778,9 +940,22 @@ cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev,
   const bool step_mode = (mode == MODE_STEP);
   const float qs = sqrtf(sqrtf(hp.c)), beta_h = hp.b / sqrtf(hp.c);
   const dim3 grid_t(kPrepBlocks, nb);
-  lt_prep<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xlo, sc.xb, sxb, sc.d0, sd, sc.ssq,
-                                        step_mode ? 1 : 0, hp.beta, hp.nesterov);
-  *launches += 1;
+  // big tiles (>= 1 M elements: the full-matrix branch, large rectangular tiles): fused ends on a grid sized by the tile
+  const bool big = (long long)g.rp * g.ldx >= (1ll << 20);
+  if (!big) {
+    lt_prep<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xlo, sc.xb, sxb, sc.d0, sd, sc.ssq,
+                                          step_mode ? 1 : 0, hp.beta, hp.nesterov);
+    *launches += 1;
+  } else {
+    if (g.transposed)
+      lt_prep_t<<<dim3((g.rp + kTP - 1) / kTP, g.ntx, nb), kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xlo, sc.xb, sxb, sc.d0,
+                                                                                sd, step_mode ? 1 : 0, hp.beta, hp.nesterov);
+    else
+      lt_prep<<<dim3(std::min(1024, (g.rp + 7) / 8), nb), kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xlo, sc.xb, sxb, sc.d0, sd,
+                                                                               nullptr, step_mode ? 1 : 0, hp.beta, hp.nesterov);
+    lt_ssq_from_d<<<nb, 1024, 0, s>>>(sc.d0, sd, g.ntx * g.rp, sc.ssq);
+    *launches += 2;
+  }
   if (hp.K > 0) {
     // Xb is double-buffered: product 3 of a step reads Xb (all rows of a column block, as the B operand of EVERY row
     // block's tile) while its epilogues write the new Xb, so input and output must be different arrays.
@@ -825,9 +1000,16 @@ cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev,
       *launches += 3;
     }
   }
-  lt_update<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, (hp.K & 1) ? sc.xb2 : sc.xb, sc.xlo, sxb,
-                                          step_mode ? 1 : 0, 1.f - hp.lr * hp.wd,
-                                          -hp.lr * hp.scale_c, 1.f / qs, hp.K == 0 ? sc.ssq : nullptr, hp.eps, qs);
+  const __nv_bfloat16* xfin = (hp.K & 1) ? sc.xb2 : sc.xb;
+  const float* ssq_fin = hp.K == 0 ? sc.ssq : nullptr;
+  if (big && g.transposed)
+    lt_update_t<<<dim3((g.rp + kTP - 1) / kTP, (g.np + kTP - 1) / kTP, nb), kEwThreads, 0, s>>>(
+        layers_dev, items_dev, g, whole, xfin, sc.xlo, sxb, step_mode ? 1 : 0, 1.f - hp.lr * hp.wd, -hp.lr * hp.scale_c, 1.f / qs, ssq_fin,
+        hp.eps, qs);
+  else
+    lt_update<<<big ? dim3((unsigned)std::min<long long>(2048, ((long long)g.rp * g.np / 8 + 2 * kEwThreads - 1) / (2 * kEwThreads)), nb) : grid_t,
+                kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, xfin, sc.xlo, sxb, step_mode ? 1 : 0, 1.f - hp.lr * hp.wd,
+                                    -hp.lr * hp.scale_c, 1.f / qs, ssq_fin, hp.eps, qs);
   *launches += 1;
   return cudaGetLastError();
 }

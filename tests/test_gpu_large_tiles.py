@@ -145,3 +145,24 @@ def test_full_matrix_branch_on_the_cta_pair_gemm(H, W):
     U2 = _run_phi(G, 1 << 20, hp)
     assert torch.equal(U1, U2)
     PU.check_phi(U1, G, max(H, W), hp, PU.TOL_TC, out_is_bf16=True)
+
+
+@pytest.mark.parametrize("H,W", [(1100, 1536), (2056, 1000)])
+def test_full_matrix_step_on_big_tiles(H, W):
+    """Full step (momentum, Nesterov, weight decay) on matrices of more than 1 M elements, wide and tall: the fused ends of
+    big tiles run on their own grid, tall ones through the shared-memory transposes (lt_prep_t / lt_update_t), here with
+    ragged last patches in both directions; two steps, the second from the stored state of the first."""
+    _need_gpu()
+    G = I.lowrank_plus_noise(H, W, 48, seed_cfg=78, layer_index=0, tensor_id=I.TENSOR_G)
+    M0 = I.lowrank_plus_noise(H, W, 48, seed_cfg=78, layer_index=0, tensor_id=I.TENSOR_M)
+    W0 = I.gaussian(H, W, seed_cfg=78, layer_index=0, tensor_id=I.TENSOR_W, dtype=torch.bfloat16, scale=0.02)
+    hp = hm.HParams(K=5, eps=1e-7, beta=0.95, nesterov=True, lr=0.02, wd=0.01, scale_c=0.2)
+    Wd, Gd, Md = W0.to(DEV), G.to(DEV), M0.to(DEV)
+    Wh, Mh = W0, M0
+    plan = hm.Plan.from_tensors([Wd], [Gd], [Md], 1 << 20).bind()
+    for _ in range(2):
+        plan.step(hp)
+        torch.cuda.synchronize()
+        PU.check_step(Wh, G, Mh, Wd.cpu(), Md.cpu(), 1 << 20, hp, PU.TOL_TC, storage_bf16=True)
+        Wh, Mh = Wd.cpu(), Md.cpu()
+    plan.destroy()

@@ -348,7 +348,7 @@ lt_update(const LayerDev* __restrict__ layers, const WorkItem* __restrict__ item
 // With one tile (or a few) per sub-batch the kPrepBlocks x nb grid of lt_prep / lt_update is a fraction of the GPU, and the
 // scalar path of a TRANSPOSED tile touches one 2-byte element per lane and row (measured on a 14336 x 4096 matrix: 6.3 ms
 // of lt_prep + 4.3 ms of lt_update beside 4.2 ms for the fifteen GEMMs).  Big tiles therefore run lt_prep / lt_update on a
-// grid sized by the tile, transposed tiles go through the two kernels below (64 x 64 patches transposed in shared
+// grid sized by the tile, transposed tiles (of any size) go through the two kernels below (64 x 64 patches transposed in shared
 // memory: every global access is a row segment in BOTH layouts), and the sum of squares of the tile comes from the d
 // partials in one fixed order (lt_ssq_from_d).
 constexpr int kTP = 64;                   // patch edge
@@ -941,8 +941,9 @@ cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev,
   const float qs = sqrtf(sqrtf(hp.c)), beta_h = hp.b / sqrtf(hp.c);
   const dim3 grid_t(kPrepBlocks, nb);
   // big tiles (>= 1 M elements: the full-matrix branch, large rectangular tiles): fused ends on a grid sized by the tile
+  // and every TRANSPOSED tile, whatever its size (rectangular tiles taller than wide), through the transposing kernels
   const bool big = (long long)g.rp * g.ldx >= (1ll << 20);
-  if (!big) {
+  if (!big && !g.transposed) {
     lt_prep<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xlo, sc.xb, sxb, sc.d0, sd, sc.ssq,
                                           step_mode ? 1 : 0, hp.beta, hp.nesterov);
     *launches += 1;
@@ -1002,7 +1003,7 @@ cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev,
   }
   const __nv_bfloat16* xfin = (hp.K & 1) ? sc.xb2 : sc.xb;
   const float* ssq_fin = hp.K == 0 ? sc.ssq : nullptr;
-  if (big && g.transposed)
+  if (g.transposed)
     lt_update_t<<<dim3((g.rp + kTP - 1) / kTP, (g.np + kTP - 1) / kTP, nb), kEwThreads, 0, s>>>(
         layers_dev, items_dev, g, whole, xfin, sc.xlo, sxb, step_mode ? 1 : 0, 1.f - hp.lr * hp.wd, -hp.lr * hp.scale_c, 1.f / qs, ssq_fin,
         hp.eps, qs);

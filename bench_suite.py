@@ -52,9 +52,15 @@ def _step_rows(args, hm, pk, dev):
                                ("llama3-8b", 16, 2048, AUTO), ("llama3-8b", 32, 2048, AUTO),
                                ("llama3-8b", 64, 2048, AUTO), ("llama3-8b", 256, 2048, AUTO), ("llama3-8b-sched", 128, 2048, AUTO),
                                ("llama3-8b", 512, 2048, AUTO), ("llama3-8b", 1 << 20, 2048, AUTO),
+                               ("llama3-8b", (128, 256), 2048, AUTO), ("llama3-8b", (256, 64), 2048, AUTO),   # rectangular (T_h, T_w)
                                ("llama3-8b", 128, 2048, FP8), ("llama3-8b", 256, 2048, FP8)):   # opt-in e4m3 operands
         spec = spec_of(name)
+        Tw = None
+        if isinstance(T, tuple):                                            # tile-shape study
+            T, Tw = T
         row = {"row": "step", "workload": name, "T": T, "cap_mb": cap}
+        if Tw:
+            row["T_w"] = Tw
         if path == FP8:
             row["path"] = "fp8 (e4m3 operands; reduced precision; peak = bf16 peak x 2)"
         try:
@@ -62,10 +68,15 @@ def _step_rows(args, hm, pk, dev):
             sets = [make_inputs(spec, dev) for _ in range(n_sets)]
             Tl = [l.T for l in spec.layers]
             plans = [hm.Plan.from_tensors(W, G, M, T, T_per_layer=Tl if any(Tl) else None, path=path,
+                                          Tw_per_layer=[Tw] * len(W) if Tw else None,
                                           workspace_cap_bytes=cap << 20).bind() for (W, G, M) in sets]
-            flops = algorithmic_flops(spec, T, args.K) if T <= 512 else float(sum(
-                6.0 * args.K * min(l.H, l.W) * l.H * l.W for l in spec.layers))   # full matrix: Gram on the short side
-            med, best = _time(lambda i: plans[i % n_sets].step(hp), args.steps if T <= 256 else 2)
+            if Tw:      # Gram matrix on the short side s of the tile: (4 s^2 l + 2 s^3) K flops per s x l tile
+                sh, lg = min(T, Tw), max(T, Tw)
+                flops = float(sum((4.0 * sh + 2.0 * sh * sh / lg) * args.K * l.H * l.W for l in spec.layers))
+            else:
+                flops = algorithmic_flops(spec, T, args.K) if T <= 512 else float(sum(
+                    6.0 * args.K * min(l.H, l.W) * l.H * l.W for l in spec.layers))   # full matrix: Gram on the short side
+            med, best = _time(lambda i: plans[i % n_sets].step(hp), args.steps if (T <= 256 and not Tw) else 2)
             bound, roof_ms = _roof(flops, 10.0 * spec.n_elements,
                                    dict(pk, bf16_sustained=2 * pk["bf16_sustained"]) if path == FP8 else pk)
             row.update({"ms": round(med, 4), "ms_min": round(best, 4), "tflops": round(flops / med / 1e9, 2),

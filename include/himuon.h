@@ -169,6 +169,11 @@ void himuon_plan_destroy(himuon_plan* plan);
  * scaled, weight-decayed parameter write entirely on chip, so every W, G, M element crosses HBM
  * once per direction. */
 himuon_status himuon_step(himuon_plan* plan, const himuon_hparams* hp, void* cuda_stream);
+/* CUDA graphs: with the plan's work list resident in its workspace (himuon_plan_info: n_chunks chunks all inside the
+ * cap, the normal case) himuon_step / himuon_phi enqueue kernel launches only, so after one eager call (which loads
+ * and configures the kernels) they may be issued under stream capture and replayed; tests/test_gpu_graph.py.  Not
+ * capturable: plans on the fp32 cuBLAS path (T >= 256 on fp32 storage / HIMUON_PATH_FP32) and plans whose work list is
+ * streamed chunk by chunk from host memory. */
 
 /* Phi_{K,T} only: w_l <- Phi_{K,T}(g_l) for every layer (no momentum, no scaling; m unused).
  * Uses hp->K, a, b, c, eps only. */

@@ -145,13 +145,24 @@ __device__ __forceinline__ TileRef tile_ref(const LayerDev* layers, const WorkIt
 }
 
 // ---- fused ends ------------------------------------------------------------------------------------------------
-// sigma = q / (||Ghat||_F + eps) of tile b from lt_prep's per-block partial sums (same order in every thread).
+// sigma = q / (||Ghat||_F + eps) of tile b from the tile's sum of squares (slot 0 of its ssq entry: lt_ssq_fold /
+// lt_ssq_from_d put it there in one fixed summation order).
+__device__ __forceinline__ float sigma_of(float tot, float eps, float qs) {
+  const float nrm = sqrtf(tot);
+  return nrm > 0.f ? qs / (nrm + eps) : 0.f;          // Phi_K(0) = 0, PAPER.md:76
+}
 __device__ __forceinline__ float tile_sigma(const float* __restrict__ ssq, int b, float eps, float qs) {
+  return sigma_of(ssq[(long long)b * kPrepBlocks], eps, qs);
+}
+// lt_prep's per-block partial sums of a tile, added in block order, into slot 0 (one thread per tile: the GEMM
+// epilogues and lt_update then need one load per tile, not kPrepBlocks of them per thread and work unit)
+__global__ void lt_ssq_fold(float* __restrict__ ssq, int nb) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= nb) return;
   float tot = 0.f;
 #pragma unroll
   for (int i = 0; i < kPrepBlocks; ++i) tot += ssq[(long long)b * kPrepBlocks + i];
-  const float nrm = sqrtf(tot);
-  return nrm > 0.f ? qs / (nrm + eps) : 0.f;          // Phi_K(0) = 0, PAPER.md:76
+  ssq[(long long)b * kPrepBlocks] = tot;
 }
 
 // 16-byte accesses of a tile: base pointers, leading dimensions and live width all multiples of 8 bf16
@@ -717,6 +728,42 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
     uint32_t nchunk = 0;                             // running chunk counter
     uint32_t xbuf = 0, xpar = 0, xprev = 0;          // E3: mirrors the producer's buffer / phase; buffer of the chunk before
     int it = 0;
+    // Row scalars of a work unit - the tile's sum of squares (first step), the d and S partials of this thread's row -
+    // are global loads with nothing to hide behind at the top of a unit (measured: 800-5800 cycles between two units of
+    // an epilogue-bound kernel).  They are therefore fetched one unit AHEAD, raw, right after the current unit's
+    // accumulator has arrived, and summed at the top of the next unit (up to two partial slots each, which covers
+    // T = 512; longer lists - big tiles, whose units are long anyway - are summed on the spot).
+    struct Raw { float tot, d0, d1, s0, s1; };
+    const bool two_slots = p.ntx <= 2 && p.ntr <= 2;
+    auto fetch = [&](long long tile) {
+      Raw r = {0.f, 0.f, 0.f, 0.f, 0.f};
+      const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
+      const int mi = rem / p.nt, ni = rem % p.nt;
+      const int i = mi * kUnitM + (int)rank * BM + row, n0 = ni * BN;
+      const bool row_ok = i < p.M;
+      if (p.ssq) r.tot = p.ssq[(long long)b * kPrepBlocks];
+      if ((EPI == EPI_X && row_ok) || (EPI == EPI_GRAM && row_ok && i >= n0 && i < n0 + BN)) {
+        const float* D = p.d_in + (long long)b * p.sd;
+        if (two_slots) {
+          r.d0 = D[i];
+          if (p.ntx > 1) r.d1 = D[(long long)p.rp + i];
+        } else {
+          for (int sl = 0; sl < p.ntx; ++sl) r.d0 += D[(long long)sl * p.rp + i];
+        }
+      }
+      if (EPI == EPI_X && row_ok) {
+        const float* S = p.s_part + (long long)b * p.ss;
+        if (two_slots) {
+          r.s0 = S[i];
+          if (p.ntr > 1) r.s1 = S[(long long)p.rp + i];
+        } else {
+          for (int sl = 0; sl < p.ntr; ++sl) r.s0 += S[(long long)sl * p.rp + i];
+        }
+      }
+      return r;
+    };
+    Raw cur = {0.f, 0.f, 0.f, 0.f, 0.f};
+    if (unit0 < n_tiles) cur = fetch(unit0);
     for (long long tile = unit0; tile < n_tiles; tile += unit_stride, ++it) {
       const int ab = it & 1;
       const int b = (int)(tile / (p.mt * p.nt)), rem = (int)(tile - (long long)b * p.mt * p.nt);
@@ -725,24 +772,16 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
       const int i = m0 + row;                        // row of C
       const bool row_ok = i < p.M;
       // first step: the iterate is the raw Ghat; sigma = q / (||Ghat||_F + eps) is applied here (header)
-      const float sig = p.ssq ? tile_sigma(p.ssq, b, p.eps, p.qs) : 1.f;
-      // row scalars, fetched before the accumulator is ready (E1 needs d_i only on the diagonal tile)
-      float d_i = 0.f, s_i = 0.f;
-      const bool has_diag = row_ok && i >= n0 && i < n0 + BN;
-      if ((EPI == EPI_X && row_ok) || (EPI == EPI_GRAM && has_diag)) {
-        const float* D = p.d_in + (long long)b * p.sd;
-        for (int sl = 0; sl < p.ntx; ++sl) d_i += D[(long long)sl * p.rp + i];
-        d_i *= sig * sig;
-      }
-      if (EPI == EPI_X && row_ok) {
-        const float* S = p.s_part + (long long)b * p.ss;
-        for (int sl = 0; sl < p.ntr; ++sl) s_i += S[(long long)sl * p.rp + i];
-        s_i = p.a + fmaf(p.beta_h, d_i, s_i);        // a + B_ii, B_ii = beta d_i + (Ah^2)_ii
-      }
+      const float sig = p.ssq ? sigma_of(cur.tot, p.eps, p.qs) : 1.f;
+      // row scalars (E1 needs d_i only on the diagonal tile; rows that need none fetched zeros)
+      float d_i = (cur.d0 + cur.d1) * (sig * sig);
+      float s_i = 0.f;
+      if (EPI == EPI_X && row_ok) s_i = p.a + fmaf(p.beta_h, d_i, cur.s0 + cur.s1);   // a + B_ii, B_ii = beta d_i + (Ah^2)_ii
       if (PAIR) mbar_wait(smem_u32(&ctrl->tfull[ab]), tph[ab]);
       else mbar_wait_parked(smem_u32(&ctrl->tfull[ab]), tph[ab]);
       tph[ab] ^= 1;
       tc_fence_after_sync();
+      const Raw nxt = tile + unit_stride < n_tiles ? fetch(tile + unit_stride) : Raw{0.f, 0.f, 0.f, 0.f, 0.f};
       const uint32_t acc = tmem_base + ab * BN + ((uint32_t)(wq * 32) << 16);
       float acc_sq = 0.f;                            // E1: sum_j ACC_ij^2; E3: sum_j x_new_ij^2 over this tile's columns
 
@@ -796,14 +835,17 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
         acc_sq = q0 + q1;
       } else {
         const float g2s = sig * sig;
-#pragma unroll 1
+        // the accumulator columns of chunk c + 1 are fetched while chunk c is converted, fenced and handed to TMA
+        uint32_t rr[2][32];
+        tmem_ld32(acc + 32 * hf, rr[0]);
+#pragma unroll
         for (int c = 0; c < BN / 64; ++c, ++nchunk) {
           const uint32_t st = epi0 + (nchunk & 1) * kEpiBuf + rsw;                // this row of the [128 x 64] bf16 chunk
           {
             const int hh = hf;
-            uint32_t r[32];
-            tmem_ld32(acc + 64 * c + 32 * hh, r);
+            uint32_t(&r)[32] = rr[c & 1];
             tmem_wait_ld();
+            if (c + 1 < BN / 64) tmem_ld32(acc + 64 * (c + 1) + 32 * hh, rr[(c + 1) & 1]);
             if (EPI == EPI_GRAM) {
 #pragma unroll
               for (int j = 0; j < 32; ++j) {
@@ -854,6 +896,7 @@ lt_gemm(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtenso
           else p.d_out[(long long)b * p.sd + (long long)ni * p.rp + i] = tot;
         }
       }
+      cur = nxt;
     }
     if (et == 0) tma_wait_group0();
   }
@@ -946,7 +989,8 @@ cudaError_t run_sub_batch(const LayerDev* layers_dev, const WorkItem* items_dev,
   if (!big && !g.transposed) {
     lt_prep<<<grid_t, kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xlo, sc.xb, sxb, sc.d0, sd, sc.ssq,
                                           step_mode ? 1 : 0, hp.beta, hp.nesterov);
-    *launches += 1;
+    lt_ssq_fold<<<(nb + 255) / 256, 256, 0, s>>>(sc.ssq, nb);
+    *launches += 2;
   } else {
     if (g.transposed)
       lt_prep_t<<<dim3((g.rp + kTP - 1) / kTP, g.ntx, nb), kEwThreads, 0, s>>>(layers_dev, items_dev, g, whole, sc.xlo, sc.xb, sxb, sc.d0,
